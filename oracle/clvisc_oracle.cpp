@@ -335,3 +335,277 @@ void limit_pi(const Oracle& o, double e, double pi[10], long* nlimit) {
   double r = o.xi * std::sqrt(e * e + 3.0 * P * P) / std::max(mag, 1e-300);
   if (r < 1.0) { for (int m = 0; m < 10; ++m) pi[m] *= r; ++*nlimit; }
 }
+
+State view(const std::vector<double>& e, const std::vector<double>* u, const std::vector<double>* pi,
+           bool use_pi) {
+  State s;
+  s.e = e.data();
+  for (int a = 0; a < 3; ++a) s.u[a] = u[a].data();
+  for (int m = 0; m < 10; ++m) s.pi[m] = use_pi ? pi[m].data() : nullptr;
+  return s;
+}
+
+// Q_T^mu = tf * T_f^{tau mu} of a state at one cell.
+void conserved_T(const Oracle& o, const State& s, size_t c, bool use_pi, double tf, double QT[4]) {
+  double P, cs2, T, Tf[4][4], ut[4];
+  eos_eval(o.eos, s.e[c], &P, &cs2, &T);
+  frame_tensor(o, s, c, use_pi, P, Tf, ut);
+  for (int m = 0; m < 4; ++m) QT[m] = tf * Tf[0][m];
+}
+
+// Bootstrap of u^{-1} (A23; "ideal hydrodynamics is employed to estimate u*^1"):
+// one ideal-fluid Euler predictor from (e, u~) with pi dropped gives u_id^1; u^{-1} = 2u^0 - u_id^1.
+void bootstrap_history(Oracle& o) {
+  const size_t N = o.N;
+  const bool milne = (o.geometry == 0);
+  State s = view(o.e, o.u, o.pi, false);
+  std::vector<double> ST[4], SP[10];
+  rhs(o, s, false, nullptr, o.tau0, ST, SP, nullptr);
+  double tf0 = milne ? o.tau0 : 1.0, tf1 = milne ? o.tau0 + o.dtau : 1.0;
+  long dummy1 = 0, dummy2 = 0;
+  for (size_t c = 0; c < N; ++c) {
+    double QT[4], M[4], e1, u1[3];
+    conserved_T(o, s, c, false, tf0, QT);
+    for (int m = 0; m < 4; ++m) M[m] = (QT[m] + o.dtau * ST[m][c]) / tf1;
+    rootfind(o, M, &e1, u1, &dummy1, &dummy2);
+    for (int a = 0; a < 3; ++a) o.uprev[a][c] = 2.0 * o.u[a][c] - u1[a];
+  }
+}
+
+// One full RK2 step n -> n+1  (Eq.49-54; readings A10-A12, A26).
+void step_once(Oracle& o) {
+  const size_t N = o.N;
+  const bool milne = (o.geometry == 0);
+  const bool visc = o.viscous();
+  const double h = o.dtau;
+  const double tau_n = o.tau0 + o.step * h, tau_1 = tau_n + h;
+  const double tf_n = milne ? tau_n : 1.0, tf_1 = milne ? tau_1 : 1.0;
+
+  // ---- stage 1 at tau_n -------------------------------------------------------------------
+  std::vector<double> dtu[4], gstar(N);
+  for (int m = 0; m < 4; ++m) dtu[m].resize(N);
+  for (size_t c = 0; c < N; ++c) {
+    double us[3], g2 = 1.0, gs2 = 1.0;
+    for (int a = 0; a < 3; ++a) {
+      us[a] = 2.0 * o.u[a][c] - o.uprev[a][c];          // u* = 2u^n - u^{n-1}
+      g2 += o.u[a][c] * o.u[a][c];
+      gs2 += us[a] * us[a];
+    }
+    gstar[c] = std::sqrt(gs2);                           // A11
+    dtu[0][c] = (gstar[c] - std::sqrt(g2)) / h;          // A10
+    for (int a = 0; a < 3; ++a) dtu[a + 1][c] = (us[a] - o.u[a][c]) / h;
+  }
+  State sn = view(o.e, o.u, o.pi, visc);
+  std::vector<double> ST[4], SP[10];
+  rhs(o, sn, visc, dtu, tau_n, ST, SP, o.cfl);
+
+  std::vector<double> e1(N), u1[3], pi1[10], QTn[4];
+  for (int a = 0; a < 3; ++a) u1[a].resize(N);
+  for (int m = 0; m < 10; ++m) pi1[m].assign(N, 0.0);
+  for (int m = 0; m < 4; ++m) QTn[m].resize(N);
+  for (size_t c = 0; c < N; ++c) {
+    double QT[4], pp[10] = {0}, M[4], uu[3];
+    conserved_T(o, sn, c, visc, tf_n, QT);
+    for (int m = 0; m < 4; ++m) QTn[m][c] = QT[m];
+    if (visc) {
+      double gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
+      for (int m = 0; m < 10; ++m) pp[m] = (gn * o.pi[m][c] + h * SP[m][c]) / gstar[c];   // Eq.49
+    }
+    for (int m = 0; m < 4; ++m) M[m] = (QT[m] + h * ST[m][c]) / tf_1 - pp[m];              // Eq.50-51
+    rootfind(o, M, &e1[c], uu, &o.n_floor, &o.n_clamp);
+    if (visc) limit_pi(o, e1[c], pp, &o.n_limit);
+    for (int a = 0; a < 3; ++a) u1[a][c] = uu[a];
+    for (int m = 0; m < 10; ++m) pi1[m][c] = pp[m];
+  }
+
+  // ---- stage 2 at tau_{n+1} ---------------------------------------------------------------
+  for (size_t c = 0; c < N; ++c) {
+    double g2 = 1.0, g12 = 1.0;
+    for (int a = 0; a < 3; ++a) { g2 += o.u[a][c] * o.u[a][c]; g12 += u1[a][c] * u1[a][c]; }
+    dtu[0][c] = (std::sqrt(g12) - std::sqrt(g2)) / h;
+    for (int a = 0; a < 3; ++a) dtu[a + 1][c] = (u1[a][c] - o.u[a][c]) / h;   // (u' - u^n)/h, A10
+  }
+  State s1 = view(e1, u1, pi1, visc);
+  std::vector<double> ST1[4], SP1[10];
+  rhs(o, s1, visc, dtu, tau_1, ST1, SP1, nullptr);
+
+  // Heun in Shu-Osher form (A26): Q^{n+1} = 1/2 [Q^n + Q(state') + h S_tot(state')], where
+  // Q(state') is rebuilt from the stored stage-1 state (after floor / clamp / limiter).
+  std::vector<double> pinew[10];
+  for (int m = 0; m < 10; ++m) pinew[m].assign(N, 0.0);
+  if (visc) {
+    for (size_t c = 0; c < N; ++c) {
+      double gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
+      double g1 = std::sqrt(1.0 + u1[0][c] * u1[0][c] + u1[1][c] * u1[1][c] + u1[2][c] * u1[2][c]);
+      for (int m = 0; m < 10; ++m)
+        pinew[m][c] = 0.5 * (gn * o.pi[m][c] + gstar[c] * pi1[m][c] + h * SP1[m][c]) / g1;   // Eq.52
+    }
+    if (o.strict_eq53) {   // Eq.53 as printed: stage-2 T source evaluated with pi^{n+1} (A12)
+      State s1b = view(e1, u1, pinew, true);
+      std::vector<double> SPdummy[10];
+      rhs(o, s1b, true, dtu, tau_1, ST1, SPdummy, nullptr);
+    }
+  }
+  for (size_t c = 0; c < N; ++c) {
+    double QT1[4], M[4], pp[10], en, uu[3];
+    conserved_T(o, s1, c, visc, tf_1, QT1);
+    for (int m = 0; m < 10; ++m) pp[m] = pinew[m][c];
+    for (int m = 0; m < 4; ++m)
+      M[m] = 0.5 * (QTn[m][c] + QT1[m] + h * ST1[m][c]) / tf_1 - pp[m];                      // Eq.53-54
+    rootfind(o, M, &en, uu, &o.n_floor, &o.n_clamp);
+    if (visc) limit_pi(o, en, pp, &o.n_limit);
+    for (int a = 0; a < 3; ++a) { o.uprev[a][c] = o.u[a][c]; o.u[a][c] = uu[a]; }
+    o.e[c] = en;
+    for (int m = 0; m < 10; ++m) o.pi[m][c] = pp[m];
+  }
+  o.e_max_seen = *std::max_element(o.e.begin(), o.e.end());
+  o.step += 1;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C ABI (host pointers, fp64, unpadded component-major SoA [comp][nz][ny][nx], x fastest).
+// ------------------------------------------------------------------------------------------
+extern "C" {
+
+void* oracle_create(int nx, int ny, int nz, double dx, double dy, double deta, const int* bc,
+                    int geometry, double dtau, double tau0, int eos_kind, int eos_n, double e_min,
+                    double e_max, const double* P, const double* T, double c_sb, double eta_over_s,
+                    double minmod_theta, double e_floor, double pi_limit_xi, double v_max,
+                    int strict_eq53) {
+  if (nx < 1 || ny < 1 || nz < 1 || !(dtau > 0)) return nullptr;
+  Oracle* o = new Oracle();
+  o->nx = nx; o->ny = ny; o->nz = nz;
+  o->d[0] = dx; o->d[1] = dy; o->d[2] = deta;
+  for (int a = 0; a < 3; ++a) o->bc[a] = bc[a];
+  o->geometry = geometry; o->dtau = dtau; o->tau0 = tau0; o->eta_s = eta_over_s;
+  o->eos.kind = eos_kind; o->eos.n = eos_n; o->eos.e_min = e_min; o->eos.e_max = e_max;
+  o->eos.c_sb = c_sb;
+  if (eos_kind == 1) { o->eos.P.assign(P, P + eos_n); o->eos.T.assign(T, T + eos_n); }
+  o->theta = minmod_theta; o->e_floor = e_floor; o->xi = pi_limit_xi; o->v_max = v_max;
+  o->strict_eq53 = strict_eq53;
+  o->N = size_t(nx) * ny * nz;
+  o->e.assign(o->N, 0.0);
+  for (int a = 0; a < 3; ++a) { o->u[a].assign(o->N, 0.0); o->uprev[a].assign(o->N, 0.0); }
+  for (int m = 0; m < 10; ++m) o->pi[m].assign(o->N, 0.0);
+  return o;
+}
+
+void oracle_destroy(void* h) { delete static_cast<Oracle*>(h); }
+
+// T: T_f^{tau mu} [4][N] (no extra factor tau); pi: pi~ [10][N] or NULL.
+int oracle_load(void* h, const double* T, const double* pi) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const size_t N = o.N;
+  for (size_t c = 0; c < N; ++c) {
+    double M[4], uu[3];
+    for (int m = 0; m < 10; ++m) o.pi[m][c] = (pi && o.viscous()) ? pi[m * N + c] : 0.0;
+    for (int m = 0; m < 4; ++m) M[m] = T[m * N + c] - o.pi[m][c];
+    rootfind(o, M, &o.e[c], uu, &o.n_floor, &o.n_clamp);
+    for (int a = 0; a < 3; ++a) o.u[a][c] = uu[a];
+  }
+  o.step = 0;
+  bootstrap_history(o);
+  o.e_max_seen = *std::max_element(o.e.begin(), o.e.end());
+  o.loaded = true;
+  return 0;
+}
+
+// Overwrite the history u~^i_{n-1} [3][N] (analytic tests that know the exact earlier level).
+int oracle_set_history(void* h, const double* uprev) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int a = 0; a < 3; ++a) std::copy(uprev + a * o.N, uprev + (a + 1) * o.N, o.uprev[a].begin());
+  return 0;
+}
+
+int oracle_step(void* h, int n) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (!o.loaded) return -4;
+  for (int s = 0; s < n; ++s) step_once(o);
+  return 0;
+}
+
+// e [N], u~^mu [4][N], pi~ [10][N]; any may be NULL.
+int oracle_read(void* h, double* e, double* u, double* pi) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const size_t N = o.N;
+  for (size_t c = 0; c < N; ++c) {
+    if (e) e[c] = o.e[c];
+    if (u) {
+      u[c] = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
+      for (int a = 0; a < 3; ++a) u[(a + 1) * N + c] = o.u[a][c];
+    }
+    if (pi) for (int m = 0; m < 10; ++m) pi[m * N + c] = o.pi[m][c];
+  }
+  return 0;
+}
+
+// T_f^{tau mu} [4][N] of the current state.
+int oracle_read_T(void* h, double* T) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  State s = view(o.e, o.u, o.pi, o.viscous());
+  for (size_t c = 0; c < o.N; ++c) {
+    double QT[4];
+    conserved_T(o, s, c, o.viscous(), 1.0, QT);
+    for (int m = 0; m < 4; ++m) T[m * o.N + c] = QT[m];
+  }
+  return 0;
+}
+
+int oracle_read_history(void* h, double* uprev) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int a = 0; a < 3; ++a) std::copy(o.uprev[a].begin(), o.uprev[a].end(), uprev + a * o.N);
+  return 0;
+}
+
+// diag[0]=tau, [1]=step, [2..4]=CFL per axis (last stage 1), [5]=e_max, [6]=floored, [7]=clamped,
+// [8]=pi-limited (cumulative counts).
+int oracle_diag(void* h, double* diag) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  diag[0] = o.tau0 + o.step * o.dtau; diag[1] = o.step;
+  for (int a = 0; a < 3; ++a) diag[2 + a] = o.cfl[a];
+  diag[5] = o.e_max_seen; diag[6] = double(o.n_floor); diag[7] = double(o.n_clamp);
+  diag[8] = double(o.n_limit);
+  return 0;
+}
+
+// RHS operator on the current state with a caller-supplied d_tau u~ [4][N] (test hook for the
+// brute-force and PDE-residual pins).  ST [4][N], SP [10][N].
+int oracle_rhs(void* h, const double* dtu, double tau, double* ST, double* SP) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const size_t N = o.N;
+  std::vector<double> d[4], st[4], sp[10];
+  for (int m = 0; m < 4; ++m) d[m].assign(dtu + m * N, dtu + (m + 1) * N);
+  State s = view(o.e, o.u, o.pi, o.viscous());
+  rhs(o, s, o.viscous(), d, tau, st, sp, nullptr);
+  for (int m = 0; m < 4; ++m) std::copy(st[m].begin(), st[m].end(), ST + m * N);
+  if (o.viscous() && SP) for (int m = 0; m < 10; ++m) std::copy(sp[m].begin(), sp[m].end(), SP + m * N);
+  return 0;
+}
+
+// Directly set the state (e [N], u~^i [3][N], pi~ [10][N] or NULL) without a root-find.
+int oracle_set_state(void* h, const double* e, const double* u, const double* pi) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const size_t N = o.N;
+  std::copy(e, e + N, o.e.begin());
+  for (int a = 0; a < 3; ++a) std::copy(u + a * N, u + (a + 1) * N, o.u[a].begin());
+  for (int m = 0; m < 10; ++m)
+    for (size_t c = 0; c < N; ++c) o.pi[m][c] = (pi && o.viscous()) ? pi[m * N + c] : 0.0;
+  o.uprev[0] = o.u[0]; o.uprev[1] = o.u[1]; o.uprev[2] = o.u[2];
+  o.step = 0; o.loaded = true;
+  return 0;
+}
+
+void oracle_eos(void* h, double e, double* out3) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  eos_eval(o.eos, e, &out3[0], &out3[1], &out3[2]);
+}
+
+void oracle_rootfind(void* h, const double* M4, double* out4) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  long a = 0, b = 0;
+  rootfind(o, M4, &out4[0], &out4[1], &a, &b);
+}
+
+}  // extern "C"

@@ -1,0 +1,105 @@
+"""Analytic / ODE references used to pin the oracle (never imported by the product or the oracle).
+
+Re-derived from PAPER.md:
+  * Bjorken: Eq.68 (:386) with the IS equation Eq.4 (:58) reduced to 0+1 D (SURVEY pin 2, A19, A20)
+  * Gubser: Weyl map Eq.70-71 (:404-409), back-map Eq.74-76 (:427-433, sign of Eq.75 per A21),
+    IS equation with lambda_i = 0 in dS3xR (SURVEY pin 3, 4)
+"""
+import math
+
+import numpy as np
+from scipy.integrate import solve_ivp
+
+HBARC = 0.1973269804
+C_SB = 47.5 * math.pi ** 2 / 30.0
+
+
+def T_conformal(e):
+    return HBARC * (e / (C_SB * HBARC)) ** 0.25
+
+
+def bjorken_is(e0, tau0, tau1, eta_s, w0=None):
+    """IS Bjorken: de/dtau = -(e+P+w)/tau, dw/dtau = -(w + 4 eta_v/(3 tau))/tau_pi - (4/3) w/tau,
+    w = pi~^{eta eta}; P = e/3.  Returns dense solution callable t -> (e, w)."""
+    def f(t, y):
+        e, w = y
+        P = e / 3.0
+        T = T_conformal(e)
+        etav = eta_s * (e + P) / T * HBARC
+        tpi = 5.0 * eta_s * HBARC / T
+        return [-(e + P + w) / t, -(w + 4 * etav / (3 * t)) / tpi - (4.0 / 3.0) * w / t]
+    if w0 is None:
+        w0 = bjorken_w_ns(e0, tau0, eta_s)
+    sol = solve_ivp(f, (tau0, tau1), [e0, w0], rtol=1e-12, atol=1e-14, dense_output=True)
+    return sol.sol
+
+
+def bjorken_w_ns(e0, tau0, eta_s):
+    """Navier-Stokes start value pi~^{eta eta} = -4 eta_v/(3 tau) (PAPER.md:384 with A20)."""
+    T0 = T_conformal(e0)
+    etav = eta_s * (4.0 * e0 / 3.0) / T0 * HBARC
+    return -4.0 * etav / (3.0 * tau0)
+
+
+class Gubser:
+    """Gubser flow for conformal IS hydro (lambda_i = 0), q = 1/L."""
+
+    def __init__(self, q=1.0, eta_s=0.2, That0=1.2, rho_range=(-6.0, 3.0)):
+        self.q, self.eta_s, self.That0 = q, eta_s, That0
+        if eta_s > 0:
+            def f(rho, y):
+                Th, wb = y
+                th = math.tanh(rho)
+                return [Th * th * (-2.0 / 3.0 + wb / 3.0),
+                        -(4.0 / 3.0) * wb * wb * th - (Th / (5.0 * eta_s)) * (wb - (4.0 / 3.0) * eta_s * th / Th)]
+            kw = dict(rtol=1e-12, atol=1e-14, dense_output=True)
+            self._neg = solve_ivp(f, (0.0, rho_range[0]), [That0, 0.0], **kw).sol
+            self._pos = solve_ivp(f, (0.0, rho_range[1]), [That0, 0.0], **kw).sol
+
+    def hat(self, rho):
+        """(T^, pibar) at rho (arrays)."""
+        rho = np.asarray(rho, dtype=np.float64)
+        if self.eta_s == 0:
+            return self.That0 * np.cosh(rho) ** (-2.0 / 3.0), np.zeros_like(rho)
+        flat = np.atleast_1d(rho).ravel()
+        out = np.empty((2, flat.size))
+        neg = flat < 0
+        if neg.any():
+            out[:, neg] = self._neg(flat[neg])
+        if (~neg).any():
+            out[:, ~neg] = self._pos(flat[~neg])
+        return out[0].reshape(rho.shape), out[1].reshape(rho.shape)
+
+    def fields(self, tau, X, Y):
+        """Returns e, u~ (4 comps: tau,x,y,eta), pi~ (10 comps) on arrays X, Y at proper time tau."""
+        q = self.q
+        r = np.sqrt(X * X + Y * Y)
+        sinh_rho = -(1.0 - q * q * tau * tau + q * q * r * r) / (2.0 * q * tau)
+        rho = np.arcsinh(sinh_rho)
+        Th, wb = self.hat(rho)
+        e = C_SB * Th ** 4 * HBARC / tau ** 4
+        vr = 2.0 * q * q * tau * r / (1.0 + q * q * tau * tau + q * q * r * r)
+        kappa = np.arctanh(vr)
+        with np.errstate(invalid="ignore", divide="ignore"):
+            nx = np.where(r > 0, X / r, 0.0)
+            ny = np.where(r > 0, Y / r, 0.0)
+        ch, sh = np.cosh(kappa), np.sinh(kappa)
+        u = np.stack([ch, sh * nx, sh * ny, np.zeros_like(r)])
+        w = (4.0 / 3.0) * e * wb            # pi~^{eta eta}
+        a = -w / 2.0
+        pi = np.zeros((10,) + r.shape)
+        pi[0] = a * sh * sh
+        pi[1] = a * sh * ch * nx
+        pi[2] = a * sh * ch * ny
+        pi[4] = a * (ch * ch * nx * nx + (1.0 - nx * nx))
+        pi[5] = a * (ch * ch * nx * ny - nx * ny)
+        pi[7] = a * (ch * ch * ny * ny + (1.0 - ny * ny))
+        pi[9] = w
+        return e, u, pi
+
+    def T_tau_mu(self, tau, X, Y):
+        """Frame tensor T_f^{tau mu} (4 comps) and pi~ for hydro_load / oracle.load."""
+        e, u, pi = self.fields(tau, X, Y)
+        P = e / 3.0
+        T = np.stack([(e + P) * u[0] * u[m] - (P if m == 0 else 0.0) + pi[m] for m in range(4)])
+        return T, pi
