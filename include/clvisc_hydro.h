@@ -1,0 +1,134 @@
+/* clvisc_hydro.h -- C ABI of the B200-native CLVisc evolution step.
+ *
+ * One call of hydro_step(ctx, 1) advances second-order viscous hydrodynamics on a
+ * (tau, x, y, eta_s) Milne grid by one RK2 (Heun) step, arXiv:1802.04449:
+ *   - KT central finite-volume update of T^{tau mu} and pi^{mu nu}   PAPER.md:193-213 (Eq.40-44)
+ *   - Israel-Stewart relaxation source of pi^{mu nu}                 PAPER.md:165-183 (Eq.33-38)
+ *   - geometric (Milne) source of T^{tau mu}                         PAPER.md:161     (Eq.31)
+ *   - root-find T^{tau mu} - pi^{tau mu} -> e, P, u^mu through the EoS  PAPER.md:229,235 (Eq.51,54)
+ *   - predictor/corrector with u* = 2u^n - u^{n-1}                   PAPER.md:225-239 (Eq.49-54)
+ * The readings of every garbled / silent passage are listed in DESIGN.md ("Readings", A1..A26).
+ *
+ * Conventions
+ *   - "tilde" (tetrad) components, g~ = diag(1,-1,-1,-1): u~ = gamma (1, v_x, v_y, v_eta),
+ *     pi~ per PAPER.md:129 (Eq.20); T_f^{tau mu} = (T^{tau tau}, T^{tau x}, T^{tau y}, tau T^{tau eta_s})
+ *     WITHOUT the paper's extra overall factor tau (Eq.18: T~ = tau * T_f).
+ *   - pi component order: 0 tt, 1 tx, 2 ty, 3 tn, 4 xx, 5 xy, 6 xn, 7 yy, 8 yn, 9 nn  (n = eta_s).
+ *   - user arrays are UNPADDED component-major SoA [comp][nz][ny][nx], x fastest, element type
+ *     double (precision 64) or float (precision 32) as chosen at create.
+ *   - every field pointer carries a memory-space tag (HYDRO_MEM_DEVICE / HYDRO_MEM_HOST).  Device
+ *     pointers are used in place, stream-ordered on opts->stream.  Host pointers are copied
+ *     through the workspace with cudaMemcpyAsync on the same stream; the call synchronises the
+ *     stream before it returns so the host buffer may be reused (pinned memory makes it fast).
+ *   - the caller owns every buffer it passes, including the workspace; the library never frees
+ *     them and keeps no pointer to field arguments after the call returns.  The workspace must
+ *     stay alive (and untouched) until hydro_destroy.
+ *   - return value: 0 success; negative = error (below); positive (hydro_step, hydro_diag) = warning
+ *     bit mask.  No exceptions, no global state; a context is not thread-safe.
+ *   - the whole path runs in CUDA kernels for sm_100a; there is no CPU fallback: without a usable
+ *     device every compute entry point returns HYDRO_ECUDA.
+ */
+#ifndef CLVISC_HYDRO_H
+#define CLVISC_HYDRO_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hydro_ctx hydro_ctx; /* opaque, owned by the library (host memory only) */
+
+enum { HYDRO_OK = 0, HYDRO_EINVAL = -1, HYDRO_ENOMEM = -2, HYDRO_ECUDA = -3, HYDRO_ESTATE = -4 };
+enum { HYDRO_WARN_CFL = 1, HYDRO_WARN_NAN = 2, HYDRO_WARN_ROOT = 4 };
+enum { HYDRO_MEM_DEVICE = 0, HYDRO_MEM_HOST = 1 };
+
+/* Grid: nx,ny,nz cells along x, y, eta_s; cell sizes in fm, fm, (unitless).
+ * bc[a]: 0 = zero-gradient outflow (neighbour index clamped; "constant extrapolation for boundary
+ * cells"), 1 = periodic.  geometry: 0 = Milne, 1 = Cartesian (all Christoffel terms
+ * off and all tau factors 1, the paper's own test mode). */
+typedef struct {
+  int nx, ny, nz;
+  double dx, dy, deta;
+  int bc[3];
+  int geometry;
+} hydro_grid;
+
+/* Equation of state.  kind 0: EOSI, P = e/3, T = hbarc (e/(c_sb hbarc))^{1/4}.
+ * kind 1: table with n log-spaced nodes e_k = e_min (e_max/e_min)^{k/(n-1)}; P and T (GeV) are HOST
+ * arrays of n doubles, copied at create; linear interpolation in e inside a bracket, c_s^2 = the
+ * slope of the bracket; below e_min P = P_0 e/e_min, T = T_0 (e/e_min)^{1/4}; above e_max
+ * P = P_{n-1} + (e-e_max)/3, T = T_{n-1} (e/e_max)^{1/4}  (A16). */
+typedef struct {
+  int kind;
+  int n;
+  double e_min, e_max;
+  const double *P, *T;
+  double c_sb;
+} hydro_eos;
+
+/* Options.  precision 64 or 32 (storage AND arithmetic).  minmod_theta in [1,2] (A4); e_floor: dynamic
+ * floor on e (A8); pi_limit_xi <= 0 switches the pi limiter off (A14); v_max: clamp of |M|/M0 (A7),
+ * <= 0 selects the default for the precision (1-1e-10 / 1-1e-6); root_iters: fixed Newton iteration
+ * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
+ * stream); workspace: DEVICE memory of at least hydro_workspace_bytes(), 256-byte aligned.
+ * kernel: 0 = default (fastest validated), 1 = reference per-cell kernel, 2 = tiled kernel. */
+typedef struct {
+  int precision;
+  double minmod_theta, e_floor, pi_limit_xi, v_max;
+  int root_iters;
+  int kernel;
+  void *stream;
+  void *workspace;
+  size_t workspace_bytes;
+} hydro_opts;
+
+/* Diagnostics (PAPER.md:640 for e_max).  cfl[a] = max over cells of
+ * c_a h / Delta_a in stage 1 of the last step; counters are cumulative since hydro_load. */
+typedef struct {
+  double tau;
+  long long step;
+  double cfl[3];
+  double e_max;
+  long long n_floor, n_clamp, n_pi_limited, n_nan, n_root_unconverged;
+} hydro_diag_t;
+
+/* Bytes of device workspace a context for this grid/precision/viscosity needs (0 on bad input). */
+size_t hydro_workspace_bytes(const hydro_grid *grid, int precision, double eta_over_s);
+
+/* Create a context.  tau0: initial proper time (fm/c), dtau: fixed step h; eta_over_s = 0 selects
+ * the ideal-fluid path (no pi array is touched, A15).  Errors: HYDRO_EINVAL (bad sizes, precision,
+ * theta, table), HYDRO_ENOMEM (workspace too small or misaligned), HYDRO_ECUDA. */
+int hydro_create(hydro_ctx **out, const hydro_grid *grid, double dtau, double tau0,
+                 const hydro_eos *eos, double eta_over_s, const hydro_opts *opts);
+
+/* Load initial data: T_tau_mu = T_f^{tau mu} [4][nz][ny][nx]; pi_mu_nu = pi~ [10][nz][ny][nx] or NULL
+ * (= 0).  Root-finds the primitives (Eq.51), bootstraps u^{-1} with one ideal-fluid predictor
+ * (A23), resets tau, step and counters.  mem: HYDRO_MEM_DEVICE / HYDRO_MEM_HOST. */
+int hydro_load(hydro_ctx *ctx, const void *T_tau_mu, const void *pi_mu_nu, int mem);
+
+/* Overwrite / read the history u~^i at step n-1, [3][nz][ny][nx] (analytic tests, bitwise resume). */
+int hydro_set_history(hydro_ctx *ctx, const void *u_prev, int mem);
+int hydro_read_history(hydro_ctx *ctx, void *u_prev, int mem);
+
+/* Advance n RK2 steps (2 kernel launches per step on opts->stream, no host synchronisation).
+ * Errors: HYDRO_ESTATE before hydro_load; HYDRO_ECUDA on a launch error. */
+int hydro_step(hydro_ctx *ctx, int n);
+
+/* Read the state: e [nz][ny][nx], u = u~^mu [4][nz][ny][nx], pi = pi~ [10][nz][ny][nx]; any may be
+ * NULL.  Synchronises the stream when mem == HYDRO_MEM_HOST. */
+int hydro_read(hydro_ctx *ctx, void *e, void *u, void *pi, int mem);
+
+/* Copy the diagnostics to the host (synchronises the stream).  Returns a warning mask. */
+int hydro_diag(hydro_ctx *ctx, hydro_diag_t *out);
+
+/* Number of kernel launches issued by this context since create (host counter). */
+long long hydro_launch_count(const hydro_ctx *ctx);
+
+void hydro_destroy(hydro_ctx *ctx);
+const char *hydro_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLVISC_HYDRO_H */

@@ -1,0 +1,510 @@
+// hydro_api.cu -- context object and C ABI (include/clvisc_hydro.h) of the B200-native CLVisc step.
+//
+// Host side only sequences launches: every arithmetic step of the path runs in the CUDA kernels of
+// hydro_stage_*.cuh / the load & read kernels below.  There is no CPU fallback.
+//
+// Workspace layout (caller-allocated device memory, 256-byte aligned pieces):
+//   [diag 256 B][EoS tables 5 x kMaxEosNodes x elem][buf A][buf B][buf X][gstar]
+// buf A/B alternate as "state n" / "state n-1 (its u~^i is the history) -> state n+1"; buf X holds the
+// stage-1 state '.  Each buf is nf fields (4 ideal, 14 viscous) of nz*ny*px elements, x fastest, the row
+// pitch px rounded up to a multiple of 8 elements so that every row starts 32-byte aligned.  buf X
+// (+gstar) doubles as the staging area for host-memory load/read between steps.
+#include "../../include/clvisc_hydro.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "hydro_stage_ref.cuh"
+#include "hydro_stage_tiled.cuh"
+
+namespace clv {
+
+constexpr int kMaxEosNodes = 1 << 16;
+constexpr double kHbarc = 0.1973269804;   // GeV fm (A18)
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  int px;
+  long long sz, sf;
+  int nf;
+  size_t elem;
+  size_t off_diag, off_eos, off_buf[3], off_gstar, total;
+};
+
+static bool make_layout(const hydro_grid* g, int precision, double eta_s, Layout* L) {
+  if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;
+  if (precision != 64 && precision != 32) return false;
+  if ((long long)g->nx * g->ny * g->nz > (1ll << 40)) return false;
+  L->elem = precision == 64 ? 8 : 4;
+  L->px = (int)align_up((size_t)g->nx, 8);
+  L->sz = (long long)g->ny * L->px;
+  L->sf = align_up((size_t)(L->sz * g->nz), 32);
+  L->nf = eta_s > 0.0 ? 14 : 4;
+  size_t off = 0;
+  L->off_diag = off; off += 256;
+  L->off_eos = off; off += align_up((size_t)5 * kMaxEosNodes * L->elem, 256);
+  for (int b = 0; b < 3; ++b) { L->off_buf[b] = off; off += align_up((size_t)L->nf * L->sf * L->elem, 256); }
+  L->off_gstar = off; off += align_up((size_t)L->sf * L->elem, 256);
+  L->total = off;
+  return true;
+}
+
+// ---------------------------------------------------------------------------------------------
+// load / read kernels (user layout: unpadded [comp][nz][ny][nx])
+// ---------------------------------------------------------------------------------------------
+template <typename R>
+struct IoArgs {
+  int nx, ny, nz, px;
+  long long sz, sf, N;
+  R e_floor, v_max;
+  EosDev<R> eos;
+  DiagDev* diag;
+};
+
+template <typename R, bool VISC>
+__global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restrict__ T, const R* __restrict__ pi,
+                                                   R* __restrict__ st) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = cu < a.N;
+  const long long cc = active ? cu : 0;
+  const int i = (int)(cc % a.nx), j = (int)((cc / a.nx) % a.ny), k = (int)(cc / ((long long)a.nx * a.ny));
+  const long long c = (long long)k * a.sz + (long long)j * a.px + i;
+  R p[10];
+#pragma unroll
+  for (int m = 0; m < 10; ++m) p[m] = (VISC && pi) ? pi[m * a.N + cc] : R(0);
+  R M[4];
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) M[mu] = T[mu * a.N + cc] - p[mu];    // T_id = T - pi  (Eq.51)
+  unsigned flags = 0;
+  R e, ux, uy, un;
+  rootfind(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, ux, uy, un, flags);
+  if (active) {
+    st[c] = e; st[a.sf + c] = ux; st[2 * a.sf + c] = uy; st[3 * a.sf + c] = un;
+    if (VISC) {
+#pragma unroll
+      for (int m = 0; m < 10; ++m) st[(F_PI + m) * a.sf + c] = p[m];
+    }
+  } else {
+    flags = 0;
+  }
+  count_flags(a.diag, flags);
+  const double r = warp_max(active ? (double)e : 0.0);
+  if ((threadIdx.x & 31) == 0) atomic_max_nonneg(&a.diag->emax[1], r);
+}
+
+template <typename R, bool VISC>
+__global__ void __launch_bounds__(256) read_kernel(IoArgs<R> a, const R* __restrict__ st, R* __restrict__ e,
+                                                   R* __restrict__ u, R* __restrict__ pi) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cu >= a.N) return;
+  const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
+  const long long c = (long long)k * a.sz + (long long)j * a.px + i;
+  if (e) e[cu] = st[c];
+  if (u) {
+    const R ux = st[a.sf + c], uy = st[2 * a.sf + c], un = st[3 * a.sf + c];
+    u[cu] = sqrt_(R(1) + ux * ux + uy * uy + un * un);
+    u[a.N + cu] = ux; u[2 * a.N + cu] = uy; u[3 * a.N + cu] = un;
+  }
+  if (pi) {
+#pragma unroll
+    for (int m = 0; m < 10; ++m) pi[m * a.N + cu] = VISC ? st[(F_PI + m) * a.sf + c] : R(0);
+  }
+}
+
+// pad (dir = 0: user -> internal) or unpad (dir = 1) three history fields
+template <typename R>
+__global__ void __launch_bounds__(256) history_kernel(IoArgs<R> a, R* __restrict__ hist, R* __restrict__ user,
+                                                      int dir) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cu >= a.N) return;
+  const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
+  const long long c = (long long)k * a.sz + (long long)j * a.px + i;
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    if (dir == 0) hist[m * a.sf + c] = user[m * a.N + cu];
+    else user[m * a.N + cu] = hist[m * a.sf + c];
+  }
+}
+
+}  // namespace clv
+
+using namespace clv;
+
+struct hydro_ctx {
+  hydro_grid grid;
+  double dtau, tau0, eta_s;
+  int precision, visc, kernel;
+  double theta, e_floor, xi, v_max;
+  int root_iters;
+  Layout L;
+  char* ws;
+  void* buf[3];
+  int cur, prev;     // indices of state n / state n-1 in buf[0..1]; buf[2] is state '
+  void* gstar;
+  DiagDev* diag;
+  EosDev<double> eos64;
+  EosDev<float> eos32;
+  cudaStream_t stream;
+  long long step;
+  long long launches;
+  bool loaded;
+};
+
+namespace {
+
+template <typename R> const EosDev<R>& eos_of(const hydro_ctx* c);
+template <> const EosDev<double>& eos_of<double>(const hydro_ctx* c) { return c->eos64; }
+template <> const EosDev<float>& eos_of<float>(const hydro_ctx* c) { return c->eos32; }
+
+template <typename R>
+int upload_eos(hydro_ctx* c, const hydro_eos* eos, EosDev<R>* q) {
+  memset(q, 0, sizeof(*q));
+  q->kind = eos->kind;
+  q->hbarc = (R)kHbarc;
+  q->conf_T_scale = (R)(1.0 / (eos->c_sb * kHbarc));
+  if (eos->kind == 0) return HYDRO_OK;
+  const int n = eos->n;
+  std::vector<double> node(n), cs2(n, 0.0), dT(n, 0.0);
+  for (int k = 0; k < n; ++k) node[k] = eos->e_min * std::pow(eos->e_max / eos->e_min, double(k) / double(n - 1));
+  for (int k = 0; k + 1 < n; ++k) {
+    cs2[k] = (eos->P[k + 1] - eos->P[k]) / (node[k + 1] - node[k]);
+    dT[k] = (eos->T[k + 1] - eos->T[k]) / (node[k + 1] - node[k]);
+  }
+  std::vector<R> h((size_t)5 * n);
+  for (int k = 0; k < n; ++k) {
+    h[k] = (R)node[k]; h[n + k] = (R)eos->P[k]; h[2 * n + k] = (R)cs2[k]; h[3 * n + k] = (R)eos->T[k];
+    h[4 * n + k] = (R)dT[k];
+  }
+  R* d = reinterpret_cast<R*>(c->ws + c->L.off_eos);
+  if (cudaMemcpyAsync(d, h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+    return HYDRO_ECUDA;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  q->n = n;
+  q->e_min = (R)node[0]; q->e_max = (R)node[n - 1];
+  q->inv_e_min = (R)(1.0 / node[0]); q->inv_e_max = (R)(1.0 / node[n - 1]);
+  q->P0_slope = (R)(eos->P[0] / eos->e_min);
+  q->P_top = (R)eos->P[n - 1]; q->T_bot = (R)eos->T[0]; q->T_top = (R)eos->T[n - 1];
+  q->log2_emin = (float)std::log2(eos->e_min);
+  q->inv_dlog2 = (float)(double(n - 1) / std::log2(eos->e_max / eos->e_min));
+  q->node = d; q->P = d + n; q->cs2 = d + 2 * n; q->T = d + 3 * n; q->dTde = d + 4 * n;
+  return HYDRO_OK;
+}
+
+template <typename R>
+IoArgs<R> io_args(const hydro_ctx* c) {
+  IoArgs<R> a;
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz; a.px = c->L.px;
+  a.sz = c->L.sz; a.sf = c->L.sf; a.N = (long long)a.nx * a.ny * a.nz;
+  a.e_floor = (R)c->e_floor; a.v_max = (R)c->v_max;
+  a.eos = eos_of<R>(c);
+  a.diag = c->diag;
+  return a;
+}
+
+template <typename R>
+StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double tau_1) {
+  StageArgs<R> a;
+  memset(&a, 0, sizeof(a));
+  const bool milne = c->grid.geometry == 0;
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz; a.px = c->L.px; a.sz = c->L.sz; a.sf = c->L.sf;
+  for (int d = 0; d < 3; ++d) a.bc[d] = c->grid.bc[d];
+  a.milne = milne ? 1 : 0;
+  a.tau = (R)tau_rhs; a.inv_tau = (R)(1.0 / tau_rhs);
+  a.tf_n = (R)(milne ? tau_n : 1.0); a.tf_1 = (R)(milne ? tau_1 : 1.0); a.inv_tf_1 = (R)(milne ? 1.0 / tau_1 : 1.0);
+  a.h = (R)c->dtau; a.inv_h = (R)(1.0 / c->dtau);
+  a.scale[0] = (R)(1.0 / c->grid.dx); a.scale[1] = (R)(1.0 / c->grid.dy);
+  a.scale[2] = (R)(milne ? 1.0 / (tau_rhs * c->grid.deta) : 1.0 / c->grid.deta);
+  a.theta = (R)c->theta; a.e_floor = (R)c->e_floor; a.xi = (R)c->xi; a.v_max = (R)c->v_max;
+  a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (5.0 * c->eta_s * kHbarc) : 0.0);
+  a.root_iters = c->root_iters;
+  a.eos = eos_of<R>(c);
+  a.diag = c->diag;
+  return a;
+}
+
+template <typename R, bool VISC, int MODE>
+int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
+  if (c->kernel == 2) {
+    launch_stage_tiled<R, VISC, MODE>(a, c->stream);
+  } else {
+    dim3 block(32, 8, 1);
+    dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, a.nz);
+    stage_ref_kernel<R, VISC, MODE><<<grid, block, 0, c->stream>>>(a);
+  }
+  c->launches += 1;
+  return cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+}
+
+template <typename R>
+int do_bootstrap(hydro_ctx* c) {
+  StageArgs<R> a = stage_args<R>(c, c->tau0, c->tau0, c->tau0 + c->dtau);
+  a.in = static_cast<const R*>(c->buf[c->cur]);
+  a.out = static_cast<R*>(c->buf[c->prev]) + c->L.sf;    // u~^i slots of the history buffer
+  a.slot = 0;
+  return launch_stage<R, false, 0>(c, a);
+}
+
+template <typename R>
+int do_step(hydro_ctx* c) {
+  const double tau_n = c->tau0 + (double)c->step * c->dtau, tau_1 = tau_n + c->dtau;
+  const int slot = (int)(c->step & 1);
+  R* cur = static_cast<R*>(c->buf[c->cur]);
+  R* prev = static_cast<R*>(c->buf[c->prev]);
+  R* X = static_cast<R*>(c->buf[2]);
+  StageArgs<R> a1 = stage_args<R>(c, tau_n, tau_n, tau_1);
+  a1.in = cur; a1.uprev = prev + c->L.sf; a1.gstar = static_cast<R*>(c->gstar); a1.out = X; a1.slot = slot;
+  StageArgs<R> a2 = stage_args<R>(c, tau_1, tau_n, tau_1);
+  a2.in = X; a2.sn = cur; a2.gstar = static_cast<R*>(c->gstar); a2.out = prev; a2.slot = slot;
+  int rc;
+  if (c->visc) {
+    rc = launch_stage<R, true, 1>(c, a1);
+    if (rc) return rc;
+    rc = launch_stage<R, true, 2>(c, a2);
+  } else {
+    rc = launch_stage<R, false, 1>(c, a1);
+    if (rc) return rc;
+    rc = launch_stage<R, false, 2>(c, a2);
+  }
+  if (rc) return rc;
+  const int t = c->cur; c->cur = c->prev; c->prev = t;
+  c->step += 1;
+  return HYDRO_OK;
+}
+
+template <typename R>
+int do_load(hydro_ctx* c, const void* T, const void* pi, int mem) {
+  const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
+  const R* dT = static_cast<const R*>(T);
+  const R* dpi = static_cast<const R*>(pi);
+  if (!c->visc) dpi = nullptr;
+  if (mem == HYDRO_MEM_HOST) {
+    R* stage = static_cast<R*>(c->buf[2]);
+    if (cudaMemcpyAsync(stage, T, (size_t)4 * N * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+    dT = stage;
+    if (dpi) {
+      if (cudaMemcpyAsync(stage + 4 * N, pi, (size_t)10 * N * sizeof(R), cudaMemcpyHostToDevice, c->stream) !=
+          cudaSuccess)
+        return HYDRO_ECUDA;
+      dpi = stage + 4 * N;
+    }
+  }
+  if (cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  c->cur = 0; c->prev = 1; c->step = 0;
+  IoArgs<R> a = io_args<R>(c);
+  const unsigned nb = (unsigned)((N + 255) / 256);
+  if (c->visc) load_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+  else load_kernel<R, false><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+  c->launches += 1;
+  if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
+  int rc = do_bootstrap<R>(c);
+  if (rc) return rc;
+  if (mem == HYDRO_MEM_HOST && cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  c->loaded = true;
+  return HYDRO_OK;
+}
+
+template <typename R>
+int do_read(hydro_ctx* c, void* e, void* u, void* pi, int mem) {
+  const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
+  IoArgs<R> a = io_args<R>(c);
+  const unsigned nb = (unsigned)((N + 255) / 256);
+  const R* st = static_cast<const R*>(c->buf[c->cur]);
+  auto run = [&](R* pe, R* pu, R* pp) -> int {
+    if (c->visc) read_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, st, pe, pu, pp);
+    else read_kernel<R, false><<<nb, 256, 0, c->stream>>>(a, st, pe, pu, pp);
+    c->launches += 1;
+    return cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+  };
+  if (mem == HYDRO_MEM_DEVICE) return run(static_cast<R*>(e), static_cast<R*>(u), static_cast<R*>(pi));
+  // host: stage each requested piece through buf X (+gstar when viscous), one D2H copy per piece
+  R* stage = static_cast<R*>(c->buf[2]);
+  int rc = HYDRO_OK;
+  if (e) {
+    if ((rc = run(stage, nullptr, nullptr))) return rc;
+    if (cudaMemcpyAsync(e, stage, (size_t)N * sizeof(R), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+  }
+  if (u) {
+    R* s = c->visc ? stage + N : stage;
+    if ((rc = run(nullptr, s, nullptr))) return rc;
+    if (cudaMemcpyAsync(u, s, (size_t)4 * N * sizeof(R), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+  }
+  if (pi) {
+    if (c->visc) {
+      // the e and u pieces occupy 5N elements of the 14 sf available; pi (10N) does not fit behind them in
+      // general, so wait for their copies to be issued in stream order and reuse the area from the start.
+      if ((rc = run(nullptr, nullptr, stage))) return rc;
+      if (cudaMemcpyAsync(pi, stage, (size_t)10 * N * sizeof(R), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+        return HYDRO_ECUDA;
+    } else {
+      if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+      memset(pi, 0, (size_t)10 * N * sizeof(R));
+    }
+  }
+  return cudaStreamSynchronize(c->stream) == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+}
+
+template <typename R>
+int do_history(hydro_ctx* c, void* user, int mem, int dir) {
+  const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
+  IoArgs<R> a = io_args<R>(c);
+  const unsigned nb = (unsigned)((N + 255) / 256);
+  R* hist = static_cast<R*>(c->buf[c->prev]) + c->L.sf;
+  R* dev = static_cast<R*>(user);
+  R* stage = static_cast<R*>(c->buf[2]);
+  if (mem == HYDRO_MEM_HOST) {
+    dev = stage;
+    if (dir == 0 &&
+        cudaMemcpyAsync(stage, user, (size_t)3 * N * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+  }
+  history_kernel<R><<<nb, 256, 0, c->stream>>>(a, hist, dev, dir);
+  c->launches += 1;
+  if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
+  if (mem == HYDRO_MEM_HOST) {
+    if (dir == 1 &&
+        cudaMemcpyAsync(user, stage, (size_t)3 * N * sizeof(R), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  }
+  return HYDRO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t hydro_workspace_bytes(const hydro_grid* grid, int precision, double eta_over_s) {
+  Layout L;
+  if (!make_layout(grid, precision, eta_over_s, &L)) return 0;
+  return L.total;
+}
+
+int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double tau0, const hydro_eos* eos,
+                 double eta_over_s, const hydro_opts* opts) {
+  if (!out) return HYDRO_EINVAL;
+  *out = nullptr;
+  if (!grid || !eos || !opts) return HYDRO_EINVAL;
+  Layout L;
+  if (!make_layout(grid, opts->precision, eta_over_s, &L)) return HYDRO_EINVAL;
+  if (!(dtau > 0.0) || !(grid->dx > 0.0) || !(grid->dy > 0.0) || !(grid->deta > 0.0)) return HYDRO_EINVAL;
+  if (grid->geometry != 0 && grid->geometry != 1) return HYDRO_EINVAL;
+  if (grid->geometry == 0 && !(tau0 > 0.0)) return HYDRO_EINVAL;
+  for (int d = 0; d < 3; ++d)
+    if (grid->bc[d] != 0 && grid->bc[d] != 1) return HYDRO_EINVAL;
+  if (!(eta_over_s >= 0.0)) return HYDRO_EINVAL;
+  if (!(opts->minmod_theta >= 1.0 && opts->minmod_theta <= 2.0)) return HYDRO_EINVAL;
+  if (!(opts->e_floor > 0.0)) return HYDRO_EINVAL;
+  if (opts->kernel < 0 || opts->kernel > 2) return HYDRO_EINVAL;
+  if (eos->kind != 0 && eos->kind != 1) return HYDRO_EINVAL;
+  if (!(eos->c_sb > 0.0)) return HYDRO_EINVAL;
+  if (eos->kind == 1) {
+    if (eos->n < 2 || eos->n > kMaxEosNodes || !eos->P || !eos->T) return HYDRO_EINVAL;
+    if (!(eos->e_min > 0.0) || !(eos->e_max > eos->e_min)) return HYDRO_EINVAL;
+    for (int k = 0; k + 1 < eos->n; ++k)
+      if (!(eos->P[k + 1] >= eos->P[k])) return HYDRO_EINVAL;   // monotone P keeps the root unique (A7)
+  }
+  if (!opts->workspace || opts->workspace_bytes < L.total || (reinterpret_cast<size_t>(opts->workspace) & 255))
+    return HYDRO_ENOMEM;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return HYDRO_ECUDA; }
+
+  hydro_ctx* c = new (std::nothrow) hydro_ctx();
+  if (!c) return HYDRO_ENOMEM;
+  c->grid = *grid; c->dtau = dtau; c->tau0 = tau0; c->eta_s = eta_over_s;
+  c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
+  c->kernel = opts->kernel == 0 ? 1 : opts->kernel;
+  c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
+  c->v_max = opts->v_max > 0.0 ? opts->v_max : (opts->precision == 64 ? 1.0 - 1e-10 : 1.0 - 1e-6);
+  c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;
+  c->L = L;
+  c->ws = static_cast<char*>(opts->workspace);
+  for (int b = 0; b < 3; ++b) c->buf[b] = c->ws + L.off_buf[b];
+  c->gstar = c->ws + L.off_gstar;
+  c->diag = reinterpret_cast<DiagDev*>(c->ws + L.off_diag);
+  c->stream = static_cast<cudaStream_t>(opts->stream);
+  c->cur = 0; c->prev = 1; c->step = 0; c->launches = 0; c->loaded = false;
+  int rc = opts->precision == 64 ? upload_eos<double>(c, eos, &c->eos64) : upload_eos<float>(c, eos, &c->eos32);
+  if (rc == HYDRO_OK && cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) rc = HYDRO_ECUDA;
+  if (rc != HYDRO_OK) { delete c; return rc; }
+  *out = c;
+  return HYDRO_OK;
+}
+
+int hydro_load(hydro_ctx* c, const void* T, const void* pi, int mem) {
+  if (!c || !T || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
+  return c->precision == 64 ? do_load<double>(c, T, pi, mem) : do_load<float>(c, T, pi, mem);
+}
+
+int hydro_set_history(hydro_ctx* c, const void* u_prev, int mem) {
+  if (!c || !u_prev || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
+  if (!c->loaded) return HYDRO_ESTATE;
+  void* p = const_cast<void*>(u_prev);
+  return c->precision == 64 ? do_history<double>(c, p, mem, 0) : do_history<float>(c, p, mem, 0);
+}
+
+int hydro_read_history(hydro_ctx* c, void* u_prev, int mem) {
+  if (!c || !u_prev || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
+  if (!c->loaded) return HYDRO_ESTATE;
+  return c->precision == 64 ? do_history<double>(c, u_prev, mem, 1) : do_history<float>(c, u_prev, mem, 1);
+}
+
+int hydro_step(hydro_ctx* c, int n) {
+  if (!c || n < 0) return HYDRO_EINVAL;
+  if (!c->loaded) return HYDRO_ESTATE;
+  for (int s = 0; s < n; ++s) {
+    const int rc = c->precision == 64 ? do_step<double>(c) : do_step<float>(c);
+    if (rc) return rc;
+  }
+  return HYDRO_OK;
+}
+
+int hydro_read(hydro_ctx* c, void* e, void* u, void* pi, int mem) {
+  if (!c || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
+  if (!c->loaded) return HYDRO_ESTATE;
+  return c->precision == 64 ? do_read<double>(c, e, u, pi, mem) : do_read<float>(c, e, u, pi, mem);
+}
+
+int hydro_diag(hydro_ctx* c, hydro_diag_t* out) {
+  if (!c || !out) return HYDRO_EINVAL;
+  DiagDev d;
+  if (cudaMemcpyAsync(&d, c->diag, sizeof(d), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  const int slot = (int)((c->step + 1) & 1);    // slot of the last completed step ((step-1)&1); load uses 1
+  auto as_double = [](unsigned long long b) { double v; memcpy(&v, &b, 8); return v; };
+  out->tau = c->tau0 + (double)c->step * c->dtau;
+  out->step = c->step;
+  for (int a = 0; a < 3; ++a) out->cfl[a] = c->step > 0 ? as_double(d.cfl[slot][a]) : 0.0;
+  out->e_max = as_double(d.emax[slot]);
+  out->n_floor = (long long)d.n_floor; out->n_clamp = (long long)d.n_clamp;
+  out->n_pi_limited = (long long)d.n_limit; out->n_nan = (long long)d.n_nan;
+  out->n_root_unconverged = (long long)d.n_unconv;
+  int warn = 0;
+  if (out->cfl[0] + out->cfl[1] + out->cfl[2] > 1.0) warn |= HYDRO_WARN_CFL;
+  if (d.n_nan) warn |= HYDRO_WARN_NAN;
+  if (d.n_unconv) warn |= HYDRO_WARN_ROOT;
+  return warn;
+}
+
+long long hydro_launch_count(const hydro_ctx* c) { return c ? c->launches : 0; }
+
+void hydro_destroy(hydro_ctx* c) { delete c; }
+
+const char* hydro_strerror(int code) {
+  switch (code) {
+    case HYDRO_OK: return "ok";
+    case HYDRO_EINVAL: return "invalid argument";
+    case HYDRO_ENOMEM: return "workspace too small or misaligned";
+    case HYDRO_ECUDA: return "CUDA error (no usable device, or a launch/copy failed)";
+    case HYDRO_ESTATE: return "call order error (hydro_load must come first)";
+    default: return code > 0 ? "warning mask" : "unknown error";
+  }
+}
+
+}  // extern "C"

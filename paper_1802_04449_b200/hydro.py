@@ -1,0 +1,239 @@
+"""Thin Python binding of the C ABI in include/clvisc_hydro.h (argument marshalling only).
+
+PyTorch supplies device memory (the workspace and the field tensors) and the CUDA stream; every step
+of the path runs in the kernels of libclvisc_hydro.so.  There is no CPU fallback: if the library is
+missing and cannot be built, or no CUDA device is usable, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from ctypes import POINTER, Structure, byref, c_double, c_int, c_longlong, c_size_t, c_void_p
+
+import numpy as np
+
+from . import build as _build
+
+HYDRO_MEM_DEVICE, HYDRO_MEM_HOST = 0, 1
+SYMBOLS = ["hydro_workspace_bytes", "hydro_create", "hydro_load", "hydro_set_history", "hydro_read_history",
+           "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_destroy", "hydro_strerror"]
+
+
+class hydro_grid(Structure):
+    _fields_ = [("nx", c_int), ("ny", c_int), ("nz", c_int), ("dx", c_double), ("dy", c_double),
+                ("deta", c_double), ("bc", c_int * 3), ("geometry", c_int)]
+
+
+class hydro_eos(Structure):
+    _fields_ = [("kind", c_int), ("n", c_int), ("e_min", c_double), ("e_max", c_double),
+                ("P", POINTER(c_double)), ("T", POINTER(c_double)), ("c_sb", c_double)]
+
+
+class hydro_opts(Structure):
+    _fields_ = [("precision", c_int), ("minmod_theta", c_double), ("e_floor", c_double),
+                ("pi_limit_xi", c_double), ("v_max", c_double), ("root_iters", c_int), ("kernel", c_int),
+                ("stream", c_void_p), ("workspace", c_void_p), ("workspace_bytes", c_size_t)]
+
+
+class hydro_diag_t(Structure):
+    _fields_ = [("tau", c_double), ("step", c_longlong), ("cfl", c_double * 3), ("e_max", c_double),
+                ("n_floor", c_longlong), ("n_clamp", c_longlong), ("n_pi_limited", c_longlong),
+                ("n_nan", c_longlong), ("n_root_unconverged", c_longlong)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libclvisc_hydro.so (building it first when stale and nvcc is present)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    lib = ctypes.CDLL(path)
+    lib.hydro_workspace_bytes.restype = c_size_t
+    lib.hydro_workspace_bytes.argtypes = [POINTER(hydro_grid), c_int, c_double]
+    lib.hydro_create.restype = c_int
+    lib.hydro_create.argtypes = [POINTER(c_void_p), POINTER(hydro_grid), c_double, c_double,
+                                 POINTER(hydro_eos), c_double, POINTER(hydro_opts)]
+    lib.hydro_load.restype = c_int
+    lib.hydro_load.argtypes = [c_void_p, c_void_p, c_void_p, c_int]
+    lib.hydro_set_history.restype = c_int
+    lib.hydro_set_history.argtypes = [c_void_p, c_void_p, c_int]
+    lib.hydro_read_history.restype = c_int
+    lib.hydro_read_history.argtypes = [c_void_p, c_void_p, c_int]
+    lib.hydro_step.restype = c_int
+    lib.hydro_step.argtypes = [c_void_p, c_int]
+    lib.hydro_read.restype = c_int
+    lib.hydro_read.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int]
+    lib.hydro_diag.restype = c_int
+    lib.hydro_diag.argtypes = [c_void_p, POINTER(hydro_diag_t)]
+    lib.hydro_launch_count.restype = c_longlong
+    lib.hydro_launch_count.argtypes = [c_void_p]
+    lib.hydro_destroy.restype = None
+    lib.hydro_destroy.argtypes = [c_void_p]
+    lib.hydro_strerror.restype = ctypes.c_char_p
+    lib.hydro_strerror.argtypes = [c_int]
+    _lib = lib
+    return lib
+
+
+class HydroError(RuntimeError):
+    pass
+
+
+def _check(rc, what):
+    if rc < 0:
+        raise HydroError(f"{what}: {load_library().hydro_strerror(rc).decode()} (rc={rc})")
+    return rc
+
+
+def make_grid(nx, ny, nz, dx, dy, deta, bc=(0, 0, 0), geometry=0):
+    g = hydro_grid()
+    g.nx, g.ny, g.nz, g.dx, g.dy, g.deta, g.geometry = nx, ny, nz, dx, dy, deta, geometry
+    g.bc[0], g.bc[1], g.bc[2] = bc
+    return g
+
+
+def workspace_bytes(grid: hydro_grid, precision: int, eta_over_s: float) -> int:
+    return int(load_library().hydro_workspace_bytes(byref(grid), precision, eta_over_s))
+
+
+class Hydro:
+    """hydro_create / hydro_load / hydro_step / hydro_read / hydro_diag / hydro_destroy.
+
+    eos: dict(kind, n, e_min, e_max, P, T, c_sb) as produced by inputs.conformal_eos() /
+    inputs.crossover_table().  Fields are torch CUDA tensors (used in place) or host arrays
+    (numpy / CPU tensors, copied inside the call), dtype float64 or float32 to match `precision`.
+    """
+
+    def __init__(self, nx, ny, nz, dx, dy, deta, dtau, tau0, eos, eta_over_s, bc=(0, 0, 0), geometry=0,
+                 precision=64, minmod_theta=1.1, e_floor=1e-7, pi_limit_xi=1.0, v_max=0.0, root_iters=0,
+                 kernel=0, device="cuda:0", stream=None):
+        import torch
+        self._torch = torch
+        self._lib = load_library()
+        self._h = c_void_p()
+        if not torch.cuda.is_available():
+            raise HydroError("no CUDA device: the CLVisc step has no CPU fallback")
+        self.device = torch.device(device)
+        self.precision = precision
+        self.dtype = torch.float64 if precision == 64 else torch.float32
+        self.np_dtype = np.float64 if precision == 64 else np.float32
+        self.shape = (nz, ny, nx)
+        self.N = nx * ny * nz
+        self.viscous = eta_over_s > 0
+        self.grid = make_grid(nx, ny, nz, dx, dy, deta, bc, geometry)
+        nbytes = workspace_bytes(self.grid, precision, eta_over_s)
+        if nbytes == 0:
+            raise HydroError("hydro_workspace_bytes: invalid grid / precision")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) // 256 * 256
+        e = hydro_eos()
+        e.kind, e.n, e.e_min, e.e_max, e.c_sb = int(eos["kind"]), int(eos["n"]), float(eos["e_min"]), \
+            float(eos["e_max"]), float(eos["c_sb"])
+        self._P = None if eos["P"] is None else np.ascontiguousarray(eos["P"], dtype=np.float64)
+        self._T = None if eos["T"] is None else np.ascontiguousarray(eos["T"], dtype=np.float64)
+        e.P = None if self._P is None else self._P.ctypes.data_as(POINTER(c_double))
+        e.T = None if self._T is None else self._T.ctypes.data_as(POINTER(c_double))
+        o = hydro_opts()
+        o.precision, o.minmod_theta, o.e_floor, o.pi_limit_xi, o.v_max = precision, minmod_theta, e_floor, \
+            pi_limit_xi, v_max
+        o.root_iters, o.kernel = root_iters, kernel
+        o.stream = c_void_p(self.stream.cuda_stream)
+        o.workspace, o.workspace_bytes = c_void_p(aligned), nbytes
+        with torch.cuda.device(self.device):
+            _check(self._lib.hydro_create(byref(self._h), byref(self.grid), dtau, tau0, byref(e), eta_over_s,
+                                          byref(o)), "hydro_create")
+
+    # -- marshalling helpers ------------------------------------------------------------------
+    def _ptr(self, a, ncomp, writable=False):
+        """(pointer, mem tag, keep-alive) of a tensor/array with ncomp*N elements of the context dtype."""
+        torch = self._torch
+        if a is None:
+            return None, HYDRO_MEM_DEVICE, None
+        if isinstance(a, torch.Tensor):
+            if a.dtype != self.dtype or not a.is_contiguous() or a.numel() != ncomp * self.N:
+                raise HydroError("tensor must be contiguous, of the context dtype, with %d elements" % (ncomp * self.N))
+            return c_void_p(a.data_ptr()), (HYDRO_MEM_DEVICE if a.is_cuda else HYDRO_MEM_HOST), a
+        a = np.ascontiguousarray(a, dtype=self.np_dtype) if not writable else a
+        if a.dtype != self.np_dtype or not a.flags["C_CONTIGUOUS"] or a.size != ncomp * self.N:
+            raise HydroError("array must be C-contiguous, of the context dtype, with %d elements" % (ncomp * self.N))
+        return c_void_p(a.ctypes.data), HYDRO_MEM_HOST, a
+
+    def load(self, T, pi=None):
+        pT, mT, kT = self._ptr(T, 4)
+        pP, mP, kP = self._ptr(pi, 10)
+        if pi is not None and mP != mT:
+            raise HydroError("T and pi must live in the same memory space")
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_load(self._h, pT, pP, mT), "hydro_load")
+
+    def set_history(self, u_prev):
+        p, m, k = self._ptr(u_prev, 3)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_set_history(self._h, p, m), "hydro_set_history")
+
+    def read_history(self, host=True):
+        out = self._empty((3,) + self.shape, host)
+        p, m, k = self._ptr(out, 3, writable=True)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_read_history(self._h, p, m), "hydro_read_history")
+        return out
+
+    def step(self, n=1):
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_step(self._h, int(n)), "hydro_step")
+
+    def _empty(self, shape, host, pinned=False):
+        torch = self._torch
+        if host:
+            return torch.empty(shape, dtype=self.dtype, pin_memory=pinned).numpy() if not pinned else \
+                torch.empty(shape, dtype=self.dtype, pin_memory=True)
+        return torch.empty(shape, dtype=self.dtype, device=self.device)
+
+    def read(self, host=True, out=None, want_pi=True):
+        """Returns (e [nz,ny,nx], u [4,...], pi [10,...]); host=True -> numpy arrays, else CUDA tensors.
+        out: optional (e, u, pi) buffers to fill (tensors or arrays in one memory space)."""
+        if out is None:
+            e = self._empty(self.shape, host)
+            u = self._empty((4,) + self.shape, host)
+            pi = self._empty((10,) + self.shape, host) if want_pi else None
+        else:
+            e, u, pi = out
+        pe, me, _ = self._ptr(e, 1, writable=True)
+        pu, mu, _ = self._ptr(u, 4, writable=True)
+        pp, mp, _ = self._ptr(pi, 10, writable=True)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_read(self._h, pe, pu, pp, me), "hydro_read")
+        return e, u, pi
+
+    def diag(self):
+        d = hydro_diag_t()
+        with self._torch.cuda.device(self.device):
+            warn = _check(self._lib.hydro_diag(self._h, byref(d)), "hydro_diag")
+        return dict(tau=d.tau, step=int(d.step), cfl=tuple(d.cfl), e_max=d.e_max, floored=int(d.n_floor),
+                    clamped=int(d.n_clamp), pi_limited=int(d.n_pi_limited), nan=int(d.n_nan),
+                    root_unconverged=int(d.n_root_unconverged), warn=warn)
+
+    def launch_count(self) -> int:
+        return int(self._lib.hydro_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.hydro_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def from_config(cfg, eos, **kw):
+    """Hydro for an inputs.Config."""
+    return Hydro(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.deta, cfg.dtau, cfg.tau0, eos, cfg.eta_over_s,
+                 bc=cfg.bc, geometry=cfg.geometry, **kw)
