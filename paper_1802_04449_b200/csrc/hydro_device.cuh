@@ -213,7 +213,9 @@ __device__ __forceinline__ void rootfind(const EosDev<R>& eos, R M0, R Mx, R My,
       const R dg = M2 * cs2 * inv * inv - R(1);
       if (g > R(0)) lo = e; else hi = e;
       R en = e - g / dg;
-      if (!(en > lo && en < hi)) en = R(0.5) * (lo + hi);
+      // the Newton step moves towards the root from the side just recorded, so it may land ON the other
+      // bracket end (root at M0 when M -> 0): accept the closed interval, bisect only outside it
+      if (!(en >= lo && en <= hi)) en = R(0.5) * (lo + hi);
       e = (abs_(g) > tol * M0) ? en : e;
     }
     {

@@ -127,18 +127,22 @@ def ic_partons(cfg: Config, seed: int = BASE_SEED + 20) -> tuple[np.ndarray, Non
     x, y, z = axes(cfg)
     T = np.zeros((4, cfg.nz, cfg.ny, cfg.nx))
     sr, sz = 0.6, 0.6
+    # windowed 1D profiles of every parton, then one (ny x n_sel) @ (n_sel x nx) product per eta plane
+    Gx = np.zeros((n, cfg.nx)); Gy = np.zeros((n, cfg.ny)); Gz = np.zeros((n, cfg.nz))
     for p in range(n):
         x0, x1, gx = _gauss_window(px[p], sr, x, cfg.dx)
         y0, y1, gy = _gauss_window(py[p], sr, y, cfg.dy)
         z0, z1, gz = _gauss_window(pz[p], sz, z, cfg.deta)
-        if gx.size == 0 or gy.size == 0 or gz.size == 0:
+        Gx[p, x0:x1] = gx; Gy[p, y0:y1] = gy; Gz[p, z0:z1] = gz / cfg.tau0
+    ptau = np.sqrt(E ** 2 + pT ** 2)
+    wts = [ptau, pT * np.cos(phi), pT * np.sin(phi)] if moving else [ptau]
+    for k in range(cfg.nz):
+        sel = np.nonzero(Gz[:, k])[0]
+        if sel.size == 0:
             continue
-        K = (gz[:, None, None] / cfg.tau0) * (gy[:, None] * gx[None, :])[None, :, :]
-        ptau = math.sqrt(E[p] ** 2 + pT[p] ** 2)
-        T[0, z0:z1, y0:y1, x0:x1] += ptau * K
-        if moving:
-            T[1, z0:z1, y0:y1, x0:x1] += (pT[p] * math.cos(phi[p])) * K
-            T[2, z0:z1, y0:y1, x0:x1] += (pT[p] * math.sin(phi[p])) * K
+        gxs, gys, gzs = Gx[sel], Gy[sel], Gz[sel, k]
+        for m, w in enumerate(wts):
+            T[m, k] = (gys * (w[sel] * gzs)[:, None]).T @ gxs
     np.maximum(T[0], 1e-6, out=T[0])
     return T, None
 
