@@ -69,7 +69,7 @@ typedef struct {
 
 /* Options.  precision 64 or 32 (storage AND arithmetic).  minmod_theta in [1,2] (A4); e_floor: dynamic
  * floor on e (A8); pi_limit_xi <= 0 switches the pi limiter off (A14); v_max: clamp of |M|/M0 (A7),
- * <= 0 selects the default for the precision (1-1e-10 / 1-1e-6); root_iters: fixed Newton iteration
+ * <= 0 selects the default 0.999 (gamma <= 22.4; A7 gives the evidence); root_iters: fixed Newton iteration
  * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
  * stream); workspace: DEVICE memory of at least hydro_workspace_bytes(), 256-byte aligned.
  * kernel: 0 = default (fastest validated), 1 = reference per-cell kernel, 2 = tiled kernel. */

@@ -66,7 +66,7 @@ class Oracle:
     """fp64 CPU oracle of the KT-RK2 viscous hydro step; same call shapes as the hydro_* C ABI."""
 
     def __init__(self, nx, ny, nz, dx, dy, deta, dtau, tau0, eos, eta_over_s, bc=(0, 0, 0),
-                 geometry=0, minmod_theta=1.1, e_floor=1e-7, pi_limit_xi=1.0, v_max=1.0 - 1e-10,
+                 geometry=0, minmod_theta=1.1, e_floor=1e-7, pi_limit_xi=1.0, v_max=0.999,
                  strict_eq53=0):
         lib = _load()
         self.shape = (nz, ny, nx)

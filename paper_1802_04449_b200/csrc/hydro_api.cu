@@ -421,7 +421,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
   c->kernel = opts->kernel == 0 ? 1 : opts->kernel;
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
-  c->v_max = opts->v_max > 0.0 ? opts->v_max : (opts->precision == 64 ? 1.0 - 1e-10 : 1.0 - 1e-6);
+  c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;
   c->L = L;
   c->ws = static_cast<char*>(opts->workspace);

@@ -34,7 +34,7 @@ def test_conservation_cartesian_periodic(conformal, eta_s):
 
 
 def test_rootfind_conformal_closed_form(conformal):
-    o = Oracle(1, 1, 1, 1, 1, 1, 0.1, 1.0, conformal, 0.0)
+    o = Oracle(1, 1, 1, 1, 1, 1, 0.1, 1.0, conformal, 0.0, v_max=1 - 1e-10)   # clamp out of the way
     rng = np.random.default_rng(3)
     for _ in range(200):
         e = 10 ** rng.uniform(-3, 2)
@@ -50,7 +50,7 @@ def test_rootfind_conformal_closed_form(conformal):
 
 
 def test_rootfind_table_roundtrip_and_clamps(crossover):
-    o = Oracle(1, 1, 1, 1, 1, 1, 0.1, 1.0, crossover, 0.0)
+    o = Oracle(1, 1, 1, 1, 1, 1, 0.1, 1.0, crossover, 0.0, v_max=1 - 1e-10)  # clamp out of the way
     rng = np.random.default_rng(4)
     for _ in range(300):
         e = 10 ** rng.uniform(-5, 3.5)          # also outside the table on both sides
@@ -63,6 +63,11 @@ def test_rootfind_table_roundtrip_and_clamps(crossover):
     assert np.allclose(o.rootfind(np.array([1e-9, 0, 0, 0])), [1e-7, 0, 0, 0])
     out = o.rootfind(np.array([1.0, 2.0, 0.0, 0.0]))
     assert np.isfinite(out).all() and out[0] >= 1e-7 and out[1] > 100
+    # default clamp v_max = 0.999 (A7): |M| is rescaled to 0.999 M0, so u^tau <= 22.4
+    o2 = Oracle(1, 1, 1, 1, 1, 1, 0.1, 1.0, crossover, 0.0)
+    out = o2.rootfind(np.array([1.0, 2.0, 0.0, 0.0]))
+    g = math.sqrt(1 + out[1] ** 2)
+    assert 15 < g <= 1 / math.sqrt(1 - 0.999 ** 2) + 1e-9 and out[2] == 0 and out[3] == 0
 
 
 def test_eos_table_matches_closed_form(crossover):
