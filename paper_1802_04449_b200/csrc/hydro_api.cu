@@ -5,6 +5,7 @@
 //
 // Workspace layout (caller-allocated device memory, 256-byte aligned pieces):
 //   [diag 256 B][EoS tables 5 x kMaxEosNodes x elem][buf A][buf B][buf X][gstar]
+// (each buf = nf evolved fields + 5 extended slots P, u^tau, c_x, c_y, c_eta used by kernel 2)
 // buf A/B alternate as "state n" / "state n-1 (its u~^i is the history) -> state n+1"; buf X holds the
 // stage-1 state '.  Each buf is nf fields (4 ideal, 14 viscous) of nz*ny*px elements, x fastest, the row
 // pitch px rounded up to a multiple of 8 elements so that every row starts 32-byte aligned.  buf X
@@ -47,7 +48,10 @@ static bool make_layout(const hydro_grid* g, int precision, double eta_s, Layout
   size_t off = 0;
   L->off_diag = off; off += 256;
   L->off_eos = off; off += align_up((size_t)5 * kMaxEosNodes * L->elem, 256);
-  for (int b = 0; b < 3; ++b) { L->off_buf[b] = off; off += align_up((size_t)L->nf * L->sf * L->elem, 256); }
+  // every state buffer carries X_COUNT extended slots (P, u^tau, c_x, c_y, c_eta) behind the nf evolved fields
+  for (int b = 0; b < 3; ++b) {
+    L->off_buf[b] = off; off += align_up((size_t)(L->nf + X_COUNT) * L->sf * L->elem, 256);
+  }
   L->off_gstar = off; off += align_up((size_t)L->sf * L->elem, 256);
   L->total = off;
   return true;
@@ -88,6 +92,14 @@ __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restr
 #pragma unroll
       for (int m = 0; m < 10; ++m) st[(F_PI + m) * a.sf + c] = p[m];
     }
+    // extended slots read by kernel 2
+    R P, cs2, cx, cy, cn;
+    eos_P(a.eos, e, P, cs2);
+    const R g = sqrt_(R(1) + ux * ux + uy * uy + un * un);
+    signal_speeds3(g, ux, uy, un, cs2, cx, cy, cn);
+    R* __restrict__ sx = st + (VISC ? 14 : 4) * a.sf;
+    sx[X_P * a.sf + c] = P; sx[X_G * a.sf + c] = g;
+    sx[X_CX * a.sf + c] = cx; sx[X_CY * a.sf + c] = cy; sx[X_CN * a.sf + c] = cn;
   } else {
     flags = 0;
   }
@@ -211,6 +223,7 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
   memset(&a, 0, sizeof(a));
   const bool milne = c->grid.geometry == 0;
   a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz; a.px = c->L.px; a.sz = c->L.sz; a.sf = c->L.sf;
+  a.xo = (long long)c->L.nf * c->L.sf;
   for (int d = 0; d < 3; ++d) a.bc[d] = c->grid.bc[d];
   a.milne = milne ? 1 : 0;
   a.tau = (R)tau_rhs; a.inv_tau = (R)(1.0 / tau_rhs);
@@ -419,7 +432,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   if (!c) return HYDRO_ENOMEM;
   c->grid = *grid; c->dtau = dtau; c->tau0 = tau0; c->eta_s = eta_over_s;
   c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
-  c->kernel = opts->kernel == 0 ? 1 : opts->kernel;
+  c->kernel = opts->kernel == 0 ? 2 : opts->kernel;
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
   c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;

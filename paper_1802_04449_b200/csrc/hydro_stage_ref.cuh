@@ -18,6 +18,7 @@ struct StageArgs {
   int nx, ny, nz;        // cells along x, y, eta_s
   int px;                // row pitch (elements)
   long long sz, sf;      // plane stride, field stride (elements)
+  long long xo;          // offset of the extended slots inside a state buffer (= nf * sf; kernel 2)
   int bc[3];             // 0 clamp (zero-gradient outflow), 1 periodic
   int milne;
   R tau, inv_tau;        // time level of this RHS evaluation
