@@ -7,9 +7,11 @@
 //   [diag 256 B][EoS tables 5 x kMaxEosNodes x elem][buf A][buf B][buf X][gstar]
 // (each buf = nf evolved fields + 5 extended slots P, u^tau, c_x, c_y, c_eta used by kernel 2)
 // buf A/B alternate as "state n" / "state n-1 (its u~^i is the history) -> state n+1"; buf X holds the
-// stage-1 state '.  Each buf is nf fields (4 ideal, 14 viscous) of nz*ny*px elements, x fastest, the row
-// pitch px rounded up to a multiple of 8 elements so that every row starts 32-byte aligned.  buf X
-// (+gstar) doubles as the staging area for host-memory load/read between steps.
+// stage-1 state '.  Each buf holds nft = nf + 5 fields (nf = 4 ideal, 14 viscous) in the blocked layout
+// [k][j][x-block][field][32]: the 32 x-consecutive cells of one field are contiguous (one 256-byte / 128-byte
+// warp transaction), and all fields of those 32 cells follow each other, so that inside a kernel the field
+// offset is a compile-time immediate and a cell's whole state lies in one 4.8 KB stretch of DRAM.
+// buf X (+gstar) doubles as the staging area for host-memory load/read between steps.
 #include "../../include/clvisc_hydro.h"
 
 #include <cmath>
@@ -29,9 +31,10 @@ constexpr double kHbarc = 0.1973269804;   // GeV fm (A18)
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
-  int px;
-  long long sz, sf;
-  int nf;
+  int nxb, blk, gp;      // x-blocks per row, elements per x-block (32 * nft), gstar row pitch
+  long long sy, sz;      // row and plane strides (elements)
+  long long nelem;       // elements of one state buffer
+  int nf, nft;
   size_t elem;
   size_t off_diag, off_eos, off_buf[3], off_gstar, total;
 };
@@ -39,20 +42,21 @@ struct Layout {
 static bool make_layout(const hydro_grid* g, int precision, double eta_s, Layout* L) {
   if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;
   if (precision != 64 && precision != 32) return false;
-  if ((long long)g->nx * g->ny * g->nz > (1ll << 40)) return false;
+  if ((long long)g->nx * g->ny * g->nz > (1ll << 36)) return false;
   L->elem = precision == 64 ? 8 : 4;
-  L->px = (int)align_up((size_t)g->nx, 8);
-  L->sz = (long long)g->ny * L->px;
-  L->sf = align_up((size_t)(L->sz * g->nz), 32);
   L->nf = eta_s > 0.0 ? 14 : 4;
+  L->nft = L->nf + X_COUNT;     // + extended slots P, u^tau, c_x, c_y, c_eta
+  L->nxb = (g->nx + 31) / 32;
+  L->blk = 32 * L->nft;
+  L->gp = 32 * L->nxb;
+  L->sy = (long long)L->nxb * L->blk;
+  L->sz = (long long)g->ny * L->sy;
+  L->nelem = (long long)g->nz * L->sz;
   size_t off = 0;
   L->off_diag = off; off += 256;
   L->off_eos = off; off += align_up((size_t)5 * kMaxEosNodes * L->elem, 256);
-  // every state buffer carries X_COUNT extended slots (P, u^tau, c_x, c_y, c_eta) behind the nf evolved fields
-  for (int b = 0; b < 3; ++b) {
-    L->off_buf[b] = off; off += align_up((size_t)(L->nf + X_COUNT) * L->sf * L->elem, 256);
-  }
-  L->off_gstar = off; off += align_up((size_t)L->sf * L->elem, 256);
+  for (int b = 0; b < 3; ++b) { L->off_buf[b] = off; off += align_up((size_t)L->nelem * L->elem, 256); }
+  L->off_gstar = off; off += align_up((size_t)g->nz * g->ny * L->gp * L->elem, 256);
   L->total = off;
   return true;
 }
@@ -62,8 +66,8 @@ static bool make_layout(const hydro_grid* g, int precision, double eta_s, Layout
 // ---------------------------------------------------------------------------------------------
 template <typename R>
 struct IoArgs {
-  int nx, ny, nz, px;
-  long long sz, sf, N;
+  int nx, ny, nz, blk;
+  long long sy, sz, N;
   R e_floor, v_max;
   EosDev<R> eos;
   DiagDev* diag;
@@ -76,7 +80,7 @@ __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restr
   const bool active = cu < a.N;
   const long long cc = active ? cu : 0;
   const int i = (int)(cc % a.nx), j = (int)((cc / a.nx) % a.ny), k = (int)(cc / ((long long)a.nx * a.ny));
-  const long long c = (long long)k * a.sz + (long long)j * a.px + i;
+  const long long c = (long long)k * a.sz + (long long)j * a.sy + xoff(i, a.blk);
   R p[10];
 #pragma unroll
   for (int m = 0; m < 10; ++m) p[m] = (VISC && pi) ? pi[m * a.N + cc] : R(0);
@@ -87,19 +91,19 @@ __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restr
   R e, ux, uy, un;
   rootfind(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, ux, uy, un, flags);
   if (active) {
-    st[c] = e; st[a.sf + c] = ux; st[2 * a.sf + c] = uy; st[3 * a.sf + c] = un;
+    st[c] = e; st[FS + c] = ux; st[2 * FS + c] = uy; st[3 * FS + c] = un;
     if (VISC) {
 #pragma unroll
-      for (int m = 0; m < 10; ++m) st[(F_PI + m) * a.sf + c] = p[m];
+      for (int m = 0; m < 10; ++m) st[(F_PI + m) * FS + c] = p[m];
     }
     // extended slots read by kernel 2
     R P, cs2, cx, cy, cn;
     eos_P(a.eos, e, P, cs2);
     const R g = sqrt_(R(1) + ux * ux + uy * uy + un * un);
     signal_speeds3(g, ux, uy, un, cs2, cx, cy, cn);
-    R* __restrict__ sx = st + (VISC ? 14 : 4) * a.sf;
-    sx[X_P * a.sf + c] = P; sx[X_G * a.sf + c] = g;
-    sx[X_CX * a.sf + c] = cx; sx[X_CY * a.sf + c] = cy; sx[X_CN * a.sf + c] = cn;
+    R* __restrict__ sx = st + (VISC ? 14 : 4) * FS + c;
+    sx[X_P * FS] = P; sx[X_G * FS] = g;
+    sx[X_CX * FS] = cx; sx[X_CY * FS] = cy; sx[X_CN * FS] = cn;
   } else {
     flags = 0;
   }
@@ -114,16 +118,16 @@ __global__ void __launch_bounds__(256) read_kernel(IoArgs<R> a, const R* __restr
   const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (cu >= a.N) return;
   const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
-  const long long c = (long long)k * a.sz + (long long)j * a.px + i;
+  const long long c = (long long)k * a.sz + (long long)j * a.sy + xoff(i, a.blk);
   if (e) e[cu] = st[c];
   if (u) {
-    const R ux = st[a.sf + c], uy = st[2 * a.sf + c], un = st[3 * a.sf + c];
+    const R ux = st[FS + c], uy = st[2 * FS + c], un = st[3 * FS + c];
     u[cu] = sqrt_(R(1) + ux * ux + uy * uy + un * un);
     u[a.N + cu] = ux; u[2 * a.N + cu] = uy; u[3 * a.N + cu] = un;
   }
   if (pi) {
 #pragma unroll
-    for (int m = 0; m < 10; ++m) pi[m * a.N + cu] = VISC ? st[(F_PI + m) * a.sf + c] : R(0);
+    for (int m = 0; m < 10; ++m) pi[m * a.N + cu] = VISC ? st[(F_PI + m) * FS + c] : R(0);
   }
 }
 
@@ -134,11 +138,11 @@ __global__ void __launch_bounds__(256) history_kernel(IoArgs<R> a, R* __restrict
   const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (cu >= a.N) return;
   const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
-  const long long c = (long long)k * a.sz + (long long)j * a.px + i;
+  const long long c = (long long)k * a.sz + (long long)j * a.sy + xoff(i, a.blk);
 #pragma unroll
   for (int m = 0; m < 3; ++m) {
-    if (dir == 0) hist[m * a.sf + c] = user[m * a.N + cu];
-    else user[m * a.N + cu] = hist[m * a.sf + c];
+    if (dir == 0) hist[m * FS + c] = user[m * a.N + cu];
+    else user[m * a.N + cu] = hist[m * FS + c];
   }
 }
 
@@ -209,8 +213,8 @@ int upload_eos(hydro_ctx* c, const hydro_eos* eos, EosDev<R>* q) {
 template <typename R>
 IoArgs<R> io_args(const hydro_ctx* c) {
   IoArgs<R> a;
-  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz; a.px = c->L.px;
-  a.sz = c->L.sz; a.sf = c->L.sf; a.N = (long long)a.nx * a.ny * a.nz;
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz; a.blk = c->L.blk;
+  a.sy = c->L.sy; a.sz = c->L.sz; a.N = (long long)a.nx * a.ny * a.nz;
   a.e_floor = (R)c->e_floor; a.v_max = (R)c->v_max;
   a.eos = eos_of<R>(c);
   a.diag = c->diag;
@@ -222,8 +226,8 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
   StageArgs<R> a;
   memset(&a, 0, sizeof(a));
   const bool milne = c->grid.geometry == 0;
-  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz; a.px = c->L.px; a.sz = c->L.sz; a.sf = c->L.sf;
-  a.xo = (long long)c->L.nf * c->L.sf;
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz;
+  a.blk = c->L.blk; a.gp = c->L.gp; a.sy = c->L.sy; a.sz = c->L.sz;
   for (int d = 0; d < 3; ++d) a.bc[d] = c->grid.bc[d];
   a.milne = milne ? 1 : 0;
   a.tau = (R)tau_rhs; a.inv_tau = (R)(1.0 / tau_rhs);
@@ -256,9 +260,9 @@ template <typename R>
 int do_bootstrap(hydro_ctx* c) {
   StageArgs<R> a = stage_args<R>(c, c->tau0, c->tau0, c->tau0 + c->dtau);
   a.in = static_cast<const R*>(c->buf[c->cur]);
-  a.out = static_cast<R*>(c->buf[c->prev]) + c->L.sf;    // u~^i slots of the history buffer
+  a.out = static_cast<R*>(c->buf[c->prev]) + FS;         // u~^i slots (fields 1..3) of the history buffer
   a.slot = 0;
-  return launch_stage<R, false, 0>(c, a);
+  return c->visc ? launch_stage<R, true, 0>(c, a) : launch_stage<R, false, 0>(c, a);
 }
 
 template <typename R>
@@ -269,7 +273,7 @@ int do_step(hydro_ctx* c) {
   R* prev = static_cast<R*>(c->buf[c->prev]);
   R* X = static_cast<R*>(c->buf[2]);
   StageArgs<R> a1 = stage_args<R>(c, tau_n, tau_n, tau_1);
-  a1.in = cur; a1.uprev = prev + c->L.sf; a1.gstar = static_cast<R*>(c->gstar); a1.out = X; a1.slot = slot;
+  a1.in = cur; a1.uprev = prev + FS; a1.gstar = static_cast<R*>(c->gstar); a1.out = X; a1.slot = slot;
   StageArgs<R> a2 = stage_args<R>(c, tau_1, tau_n, tau_1);
   a2.in = X; a2.sn = cur; a2.gstar = static_cast<R*>(c->gstar); a2.out = prev; a2.slot = slot;
   int rc;
@@ -368,7 +372,7 @@ int do_history(hydro_ctx* c, void* user, int mem, int dir) {
   const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
   IoArgs<R> a = io_args<R>(c);
   const unsigned nb = (unsigned)((N + 255) / 256);
-  R* hist = static_cast<R*>(c->buf[c->prev]) + c->L.sf;
+  R* hist = static_cast<R*>(c->buf[c->prev]) + FS;
   R* dev = static_cast<R*>(user);
   R* stage = static_cast<R*>(c->buf[2]);
   if (mem == HYDRO_MEM_HOST) {

@@ -16,9 +16,11 @@ namespace clv {
 template <typename R>
 struct StageArgs {
   int nx, ny, nz;        // cells along x, y, eta_s
-  int px;                // row pitch (elements)
-  long long sz, sf;      // plane stride, field stride (elements)
-  long long xo;          // offset of the extended slots inside a state buffer (= nf * sf; kernel 2)
+  // state-buffer layout [k][j][x-block][field][32]: element (field m, cell i,j,k) sits at
+  //   k*sz + j*sy + (i>>5)*blk + m*32 + (i&31);   blk = 32 * (fields per buffer)
+  int blk;               // elements per x-block (32 cells x all fields of the buffer)
+  int gp;                // row pitch of the single-field gstar array (= 32 * x-blocks)
+  long long sy, sz;      // row stride, plane stride (elements)
   int bc[3];             // 0 clamp (zero-gradient outflow), 1 periodic
   int milne;
   R tau, inv_tau;        // time level of this RHS evaluation
@@ -39,9 +41,24 @@ struct StageArgs {
   int slot;              // parity slot of the per-step maxima
 };
 
+constexpr int FS = 32;   // field stride inside an x-block (elements)
+
 __device__ __forceinline__ int bmap(int i, int n, int periodic) {
   if (periodic) { i = i % n; return i < 0 ? i + n : i; }
   return min(max(i, 0), n - 1);
+}
+__device__ __forceinline__ long long xoff(int i, int blk) { return (long long)(i >> 5) * blk + (i & 31); }
+// offsets of the five points pos-2..pos+2 along axis ax through cell (i,j,k), boundary rule a11 applied
+template <typename A>
+__device__ __forceinline__ void star_offsets(const A& a, int ax, int i, int j, int k, long long idx[5]) {
+#pragma unroll
+  for (int p = 0; p < 5; ++p) {
+    const int d = p - 2;
+    const int ii = ax == 0 ? bmap(i + d, a.nx, a.bc[0]) : i;
+    const int jj = ax == 1 ? bmap(j + d, a.ny, a.bc[1]) : j;
+    const int kk = ax == 2 ? bmap(k + d, a.nz, a.bc[2]) : k;
+    idx[p] = (long long)kk * a.sz + (long long)jj * a.sy + xoff(ii, a.blk);
+  }
 }
 
 template <typename R, bool VISC, int MODE>
@@ -51,9 +68,10 @@ __global__ void __launch_bounds__(256) stage_ref_kernel(const StageArgs<R> a) {
   const int k = blockIdx.z;
   const bool active = (i < a.nx) && (j < a.ny);
   const int ic = active ? i : 0, jc = active ? j : 0;
-  const long long c = (long long)k * a.sz + (long long)jc * a.px + ic;
+  const long long c = (long long)k * a.sz + (long long)jc * a.sy + xoff(ic, a.blk);
+  const long long cg = ((long long)k * a.ny + jc) * a.gp + ic;      // gstar index
   const R* __restrict__ in = a.in;
-  const long long sf = a.sf;
+  constexpr long long sf = FS;
   constexpr bool USE_PI = VISC && (MODE != 0);
 
   // ---- cell-centre state -------------------------------------------------------------------
@@ -80,13 +98,8 @@ __global__ void __launch_bounds__(256) stage_ref_kernel(const StageArgs<R> a) {
   // ---- KT flux divergence, axes x, y, eta in this order (Eq.40; A22) ---------------------------
 #pragma unroll 1
   for (int ax = 0; ax < 3; ++ax) {
-    const int n_ax = ax == 0 ? a.nx : (ax == 1 ? a.ny : a.nz);
-    const int pos = ax == 0 ? ic : (ax == 1 ? jc : k);
-    const long long stride = ax == 0 ? 1 : (ax == 1 ? (long long)a.px : a.sz);
-    const long long base = c - (long long)pos * stride;
     long long idx[5];
-#pragma unroll
-    for (int p = 0; p < 5; ++p) idx[p] = base + (long long)bmap(pos + p - 2, n_ax, a.bc[ax]) * stride;
+    star_offsets(a, ax, ic, jc, k, idx);
 
     R w[5], Pp[5], g[5], ux[5], uy[5], un[5], ua[5], cs[5];
 #pragma unroll
@@ -187,7 +200,7 @@ __global__ void __launch_bounds__(256) stage_ref_kernel(const StageArgs<R> a) {
       grad[0][1] = (sx - ut[1]) * a.inv_h; grad[0][2] = (sy - ut[2]) * a.inv_h; grad[0][3] = (sn_ - ut[3]) * a.inv_h;
       gdiv = gst;
     } else {
-      gst = a.gstar[c];
+      gst = a.gstar[cg];
       const R g12 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
       const R gn2 = R(1) + un_[1] * un_[1] + un_[2] * un_[2] + un_[3] * un_[3];
       grad[0][0] = (g12 - gn2) / (ut[0] + un_[0]) * a.inv_h;
@@ -250,7 +263,7 @@ __global__ void __launch_bounds__(256) stage_ref_kernel(const StageArgs<R> a) {
       if (VISC) {
 #pragma unroll
         for (int m = 0; m < 10; ++m) out[(F_PI + m) * sf + c] = pnew[m];
-        if (MODE == 1) a.gstar[c] = gst;
+        if (MODE == 1) a.gstar[cg] = gst;
       }
     }
   }

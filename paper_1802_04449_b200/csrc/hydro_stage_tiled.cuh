@@ -28,12 +28,24 @@ __device__ __forceinline__ float fabs_(float x) { return fabsf(x); }
 __device__ __forceinline__ double fmin_(double a, double b) { return fmin(a, b); }
 __device__ __forceinline__ float fmin_(float a, float b) { return fminf(a, b); }
 
-// minmod(theta dm, (dm+dp)/2, theta dp) = sign * min(theta min(|dm|,|dp|), |dm+dp|/2) when dm, dp share a sign
-template <typename R>
-__device__ __forceinline__ R minmod_fast(R dm, R dp, R theta) {
-  const R m1 = fmin_(fabs_(dm), fabs_(dp));
-  const R m = fmin_(theta * m1, R(0.5) * fabs_(dm + dp));
-  return same_sign(dm, dp) ? copysign_(m, dm) : R(0);
+// hmm(dm, dp) = 1/2 minmod(theta dm, (dm+dp)/2, theta dp)
+//             = 1/2 sign(dm) min(theta min(|dm|,|dp|), |dm+dp|/2) when dm, dp share a sign, else 0.
+// Written so that ptxas emits 5 fp64 instructions (2 DSETP, DADD, 2 DMUL) + 1 DMUL for the signed 1/2 and 8
+// integer-pipe instructions; plain fmin() costs twice that (NaN quieting and register moves).
+__device__ __forceinline__ double hmm(double dm, double dp, double theta) {
+  const double s = fabs(dm) < fabs(dp) ? dm : dp;
+  const double t = fabs(s) * theta;
+  const double h = fabs(dm + dp) * 0.5;
+  const double m = t < h ? t : h;
+  const int hm = __double2hiint(dm), hp = __double2hiint(dp);
+  const int khi = ((hm ^ hp) >= 0) ? (0x3fe00000 | (hm & 0x80000000)) : 0;     // +-0.5 or 0
+  return m * __hiloint2double(khi, 0);
+}
+__device__ __forceinline__ float hmm(float dm, float dp, float theta) {
+  const float m = fminf(theta * fminf(fabsf(dm), fabsf(dp)), 0.5f * fabsf(dm + dp));
+  const int hm = __float_as_int(dm), hp = __float_as_int(dp);
+  const int k = ((hm ^ hp) >= 0) ? (0x3f000000 | (hm & 0x80000000)) : 0;       // +-0.5f or 0
+  return m * __int_as_float(k);
 }
 
 // 2 (H_{i+1/2} - H_{i-1/2}) for one field (the factor 1/2 of Eq.41 is folded into the caller's scale)
@@ -41,10 +53,8 @@ template <typename R>
 __device__ __forceinline__ R kt_div2(const R q[5], const R f[5], R cl, R cr, R theta) {
   const R dq0 = q[1] - q[0], dq1 = q[2] - q[1], dq2 = q[3] - q[2], dq3 = q[4] - q[3];
   const R df0 = f[1] - f[0], df1 = f[2] - f[1], df2 = f[3] - f[2], df3 = f[4] - f[3];
-  const R hq1 = R(0.5) * minmod_fast(dq0, dq1, theta), hq2 = R(0.5) * minmod_fast(dq1, dq2, theta),
-          hq3 = R(0.5) * minmod_fast(dq2, dq3, theta);
-  const R hf1 = R(0.5) * minmod_fast(df0, df1, theta), hf2 = R(0.5) * minmod_fast(df1, df2, theta),
-          hf3 = R(0.5) * minmod_fast(df2, df3, theta);
+  const R hq1 = hmm(dq0, dq1, theta), hq2 = hmm(dq1, dq2, theta), hq3 = hmm(dq2, dq3, theta);
+  const R hf1 = hmm(df0, df1, theta), hf2 = hmm(df1, df2, theta), hf3 = hmm(df2, df3, theta);
   const R Hr = ((f[3] - hf3) + (f[2] + hf2)) - cr * ((q[3] - hq3) - (q[2] + hq2));
   const R Hl = ((f[2] - hf2) + (f[1] + hf1)) - cl * ((q[2] - hq2) - (q[1] + hq1));
   return Hr - Hl;
@@ -140,109 +150,127 @@ __device__ __forceinline__ void limit_pi_P(R xi, R e, R P, R pi[10], unsigned& f
 template <typename R, bool VISC, int MODE>
 __global__ void __launch_bounds__(256, 2) stage_fused_kernel(const StageArgs<R> a) {
   constexpr bool USE_PI = VISC && (MODE != 0);
+  constexpr int NF = VISC ? 14 : 4;                 // evolved fields of a buffer; extended slots follow
+  constexpr int OX = NF * FS;                       // element offset of the extended slots inside an x-block
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
   const bool active = (i < a.nx) && (j < a.ny);
   const int ic = active ? i : 0, jc = active ? j : 0;
-  const long long sf = a.sf;
-  const long long c = (long long)k * a.sz + (long long)jc * a.px + ic;
+  constexpr int sf = FS;
+  const long long c = (long long)k * a.sz + (long long)jc * a.sy + xoff(ic, a.blk);
+  const long long cg = ((long long)k * a.ny + jc) * a.gp + ic;
   const R* __restrict__ in = a.in;
-  const R* __restrict__ inx = a.in + a.xo;                  // extended slots of the input state
+  const R* __restrict__ pc = a.in + c;              // this cell: field m at pc[m * FS] (immediate offsets)
 
-  // ---- cell-centre state ------------------------------------------------------------------------
-  const R e_c = in[c];
-  R ut[4];
-  ut[1] = in[sf + c]; ut[2] = in[2 * sf + c]; ut[3] = in[3 * sf + c];
-  ut[0] = inx[X_G * sf + c];
-  const R P_c = inx[X_P * sf + c];
-  R pic[10];
-#pragma unroll
-  for (int m = 0; m < 10; ++m) pic[m] = USE_PI ? in[(F_PI + m) * sf + c] : R(0);
-
+  // S_KT of the ten pi fields accumulates in thread-private shared-memory slots, so that the pi-field loop
+  // can stay rolled (its ~200-instruction body then lives in the L0 instruction cache)
+  __shared__ R sS[USE_PI ? 10 * 256 : 1];
+  const int tid = threadIdx.y * 32 + threadIdx.x;
   R S[14];
 #pragma unroll
   for (int m = 0; m < 14; ++m) S[m] = R(0);
-  R grad[4][4];
-#pragma unroll
-  for (int m = 0; m < 4; ++m)
-#pragma unroll
-    for (int n = 0; n < 4; ++n) grad[m][n] = R(0);
   R cfl0 = R(0), cfl1 = R(0), cfl2 = R(0);
   const R tf = a.milne ? a.tau : R(1);
 
   // ---- KT flux divergence, axes x, y, eta (Eq.40; A22) -------------------------------------------
 #pragma unroll 1
   for (int ax = 0; ax < 3; ++ax) {
-    const int n_ax = ax == 0 ? a.nx : (ax == 1 ? a.ny : a.nz);
-    const int pos = ax == 0 ? ic : (ax == 1 ? jc : k);
-    const long long stride = ax == 0 ? 1 : (ax == 1 ? (long long)a.px : a.sz);
-    const long long base = c - (long long)pos * stride;
     long long idx[5];
+    star_offsets(a, ax, ic, jc, k, idx);
+    const R* __restrict__ pp[5];
 #pragma unroll
-    for (int p = 0; p < 5; ++p) idx[p] = base + (long long)bmap(pos + p - 2, n_ax, a.bc[ax]) * stride;
-    const R* __restrict__ cax = inx + (X_CX + ax) * sf;   // signal speed along this axis
-    const R* __restrict__ uax = in + (1 + ax) * sf;        // u~^a
+    for (int p = 0; p < 5; ++p) pp[p] = in + idx[p];
+    const int o_ua = (1 + ax) * FS, o_ca = OX + (X_CX + ax) * FS;
 
     R g[5], ua[5];
     R cl, cr;
     {
-      const R c1 = cax[idx[1]], c2 = cax[idx[2]], c3 = cax[idx[3]];
+      const R c1 = pp[1][o_ca], c2 = pp[2][o_ca], c3 = pp[3][o_ca];
       cl = max_(c1, c2); cr = max_(c2, c3);
       const R cv = c2 * a.h * a.scale[ax];
       if (ax == 0) cfl0 = cv; else if (ax == 1) cfl1 = cv; else cfl2 = cv;
     }
 #pragma unroll
-    for (int p = 0; p < 5; ++p) { g[p] = inx[X_G * sf + idx[p]]; ua[p] = uax[idx[p]]; }
+    for (int p = 0; p < 5; ++p) { g[p] = pp[p][OX + X_G * FS]; ua[p] = pp[p][o_ua]; }
     const R sc_pi = R(0.5) * a.scale[ax], sc_T = sc_pi * tf;
 
     {
       // T fields: Q^mu/tau = T_f^{tau mu}, F_a^mu/tau = T_f^{a mu}   (Eq.27, Eq.39)
-      R wq[5], wa[5], Pp[5], uu[3][5];
+      R wq[5], wa[5], Pp[5];
 #pragma unroll
       for (int p = 0; p < 5; ++p) {
-        Pp[p] = inx[X_P * sf + idx[p]];
-        const R w = in[idx[p]] + Pp[p];
+        Pp[p] = pp[p][OX + X_P * FS];
+        const R w = pp[p][0] + Pp[p];
         wq[p] = w * g[p]; wa[p] = w * ua[p];
-        uu[0][p] = in[sf + idx[p]]; uu[1][p] = in[2 * sf + idx[p]]; uu[2][p] = in[3 * sf + idx[p]];
       }
 #pragma unroll
       for (int mu = 0; mu < 4; ++mu) {
         R q[5], f[5];
-        const R* __restrict__ pt = in + (F_PI + c_pidx[0][mu]) * sf;
-        const R* __restrict__ pa = in + (F_PI + c_pidx[ax + 1][mu]) * sf;
+        const int o_t = (F_PI + (mu == 0 ? 0 : mu)) * FS;            // pi^{tau mu}: components 0..3
+        const int o_a = (F_PI + c_pidx[ax + 1][mu]) * FS;            // pi^{a mu}
 #pragma unroll
         for (int p = 0; p < 5; ++p) {
-          const R umu = mu == 0 ? g[p] : uu[mu == 0 ? 0 : mu - 1][p];
+          const R umu = mu == 0 ? g[p] : pp[p][mu * FS];
           R tq = wq[p] * umu - (mu == 0 ? Pp[p] : R(0));
           R tfl = wa[p] * umu + (mu == ax + 1 ? Pp[p] : R(0));
-          if (USE_PI) { tq += pt[idx[p]]; tfl += pa[idx[p]]; }
+          if (USE_PI) { tq += pp[p][o_t]; tfl += pp[p][o_a]; }
           q[p] = tq; f[p] = tfl;
         }
         S[mu] -= kt_div2(q, f, cl, cr, a.theta) * sc_T;
       }
-      if (USE_PI) {
-        // spatial rows of nabla~_mu u~^nu by central differences (A9); eta row divided by tau (Eq.22)
-        const R d0 = (g[3] - g[1]) * sc_pi, d1 = (uu[0][3] - uu[0][1]) * sc_pi, d2 = (uu[1][3] - uu[1][1]) * sc_pi,
-                d3 = (uu[2][3] - uu[2][1]) * sc_pi;
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-          if (ax == r) { grad[r + 1][0] = d0; grad[r + 1][1] = d1; grad[r + 1][2] = d2; grad[r + 1][3] = d3; }
-      }
     }
     // pi fields: Q = u^tau pi, F_a = u^a pi   (Eq.29)
     if (USE_PI) {
-#pragma unroll
-      for (int m = 0; m < 10; ++m) {
-        const R* __restrict__ pm = in + (F_PI + m) * sf;
+      int om = F_PI * FS;
+#pragma unroll 1
+      for (int m = 0; m < 10; ++m, om += FS) {
         R q[5], f[5];
 #pragma unroll
         for (int p = 0; p < 5; ++p) {
-          const R v = pm[idx[p]];
+          const R v = pp[p][om];
           q[p] = g[p] * v; f[p] = ua[p] * v;
         }
-        S[4 + m] -= kt_div2(q, f, cl, cr, a.theta) * sc_pi;
+        const R d = kt_div2(q, f, cl, cr, a.theta) * sc_pi;
+        R* slot = &sS[m * 256 + tid];
+        *slot = (ax == 0) ? -d : *slot - d;
       }
+    }
+  }
+  if (USE_PI) {
+#pragma unroll
+    for (int m = 0; m < 10; ++m) S[4 + m] = sS[m * 256 + tid];
+  }
+
+  // ---- cell-centre state (re-read after the flux loop: L1 hits, keeps the loop's register set small) ---
+  const R e_c = pc[0];
+  R ut[4];
+  ut[1] = pc[sf]; ut[2] = pc[2 * sf]; ut[3] = pc[3 * sf];
+  ut[0] = pc[OX + X_G * FS];
+  const R P_c = pc[OX + X_P * FS];
+  R pic[10];
+#pragma unroll
+  for (int m = 0; m < 10; ++m) pic[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
+
+  // spatial rows of nabla~_mu u~^nu by central differences (A9); eta row divided by tau (Eq.22)
+  R grad[4][4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m)
+#pragma unroll
+    for (int n = 0; n < 4; ++n) grad[m][n] = R(0);
+  if (USE_PI) {
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) {
+      const int im = ax == 0 ? bmap(ic - 1, a.nx, a.bc[0]) : ic, ip = ax == 0 ? bmap(ic + 1, a.nx, a.bc[0]) : ic;
+      const int jm = ax == 1 ? bmap(jc - 1, a.ny, a.bc[1]) : jc, jp = ax == 1 ? bmap(jc + 1, a.ny, a.bc[1]) : jc;
+      const int km = ax == 2 ? bmap(k - 1, a.nz, a.bc[2]) : k, kp = ax == 2 ? bmap(k + 1, a.nz, a.bc[2]) : k;
+      const R* __restrict__ qm = in + ((long long)km * a.sz + (long long)jm * a.sy + xoff(im, a.blk));
+      const R* __restrict__ qp = in + ((long long)kp * a.sz + (long long)jp * a.sy + xoff(ip, a.blk));
+      const R sc = R(0.5) * a.scale[ax];
+      grad[ax + 1][0] = (qp[OX + X_G * FS] - qm[OX + X_G * FS]) * sc;
+      grad[ax + 1][1] = (qp[sf] - qm[sf]) * sc;
+      grad[ax + 1][2] = (qp[2 * sf] - qm[2 * sf]) * sc;
+      grad[ax + 1][3] = (qp[3 * sf] - qm[3 * sf]) * sc;
     }
   }
 
@@ -258,20 +286,20 @@ __global__ void __launch_bounds__(256, 2) stage_fused_kernel(const StageArgs<R> 
 #pragma unroll
   for (int m = 0; m < 10; ++m) pin[m] = pic[m];
   if (MODE == 2) {
-    const R* __restrict__ sn = a.sn;
-    e_n = sn[c];
-    un_[1] = sn[sf + c]; un_[2] = sn[2 * sf + c]; un_[3] = sn[3 * sf + c];
-    un_[0] = sn[a.xo + X_G * sf + c];
-    P_n = sn[a.xo + X_P * sf + c];
+    const R* __restrict__ sn = a.sn + c;
+    e_n = sn[0];
+    un_[1] = sn[sf]; un_[2] = sn[2 * sf]; un_[3] = sn[3 * sf];
+    un_[0] = sn[OX + X_G * FS];
+    P_n = sn[OX + X_P * FS];
 #pragma unroll
-    for (int m = 0; m < 10; ++m) pin[m] = VISC ? sn[(F_PI + m) * sf + c] : R(0);
+    for (int m = 0; m < 10; ++m) pin[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
   }
 
   R gdiv = R(1), gst = R(1);
   if (USE_PI) {
     if (MODE == 1) {
-      const R* __restrict__ up = a.uprev;
-      const R sx = R(2) * ut[1] - up[c], sy = R(2) * ut[2] - up[sf + c], sn_ = R(2) * ut[3] - up[2 * sf + c];
+      const R* __restrict__ up = a.uprev + c;
+      const R sx = R(2) * ut[1] - up[0], sy = R(2) * ut[2] - up[sf], sn_ = R(2) * ut[3] - up[2 * sf];
       const R gs2 = R(1) + sx * sx + sy * sy + sn_ * sn_;
       gst = sqrt_(gs2);
       const R g2 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
@@ -279,7 +307,7 @@ __global__ void __launch_bounds__(256, 2) stage_fused_kernel(const StageArgs<R> 
       grad[0][1] = (sx - ut[1]) * a.inv_h; grad[0][2] = (sy - ut[2]) * a.inv_h; grad[0][3] = (sn_ - ut[3]) * a.inv_h;
       gdiv = gst;
     } else {
-      gst = a.gstar[c];
+      gst = a.gstar[cg];
       const R g12 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
       const R gn2 = R(1) + un_[1] * un_[1] + un_[2] * un_[2] + un_[3] * un_[3];
       grad[0][0] = (g12 - gn2) / (ut[0] + un_[0]) * a.inv_h;
@@ -331,21 +359,20 @@ __global__ void __launch_bounds__(256, 2) stage_fused_kernel(const StageArgs<R> 
 
   // ---- write state + extended slots ----------------------------------------------------------------
   if (active) {
-    R* __restrict__ out = a.out;
+    R* __restrict__ out = a.out + c;
     if (MODE == 0) {
-      out[c] = R(2) * ut[1] - ux_new; out[sf + c] = R(2) * ut[2] - uy_new; out[2 * sf + c] = R(2) * ut[3] - un_new;
+      out[0] = R(2) * ut[1] - ux_new; out[sf] = R(2) * ut[2] - uy_new; out[2 * sf] = R(2) * ut[3] - un_new;
     } else {
       R cx, cy, cn;
       signal_speeds3(g_new, ux_new, uy_new, un_new, cs2_new, cx, cy, cn);
-      out[c] = e_new; out[sf + c] = ux_new; out[2 * sf + c] = uy_new; out[3 * sf + c] = un_new;
+      out[0] = e_new; out[sf] = ux_new; out[2 * sf] = uy_new; out[3 * sf] = un_new;
       if (VISC) {
 #pragma unroll
-        for (int m = 0; m < 10; ++m) out[(F_PI + m) * sf + c] = pnew[m];
-        if (MODE == 1) a.gstar[c] = gst;
+        for (int m = 0; m < 10; ++m) out[(F_PI + m) * FS] = pnew[m];
+        if (MODE == 1) a.gstar[cg] = gst;
       }
-      R* __restrict__ ox = out + a.xo;
-      ox[X_P * sf + c] = P_new; ox[X_G * sf + c] = g_new;
-      ox[X_CX * sf + c] = cx; ox[X_CY * sf + c] = cy; ox[X_CN * sf + c] = cn;
+      out[OX + X_P * FS] = P_new; out[OX + X_G * FS] = g_new;
+      out[OX + X_CX * FS] = cx; out[OX + X_CY * FS] = cy; out[OX + X_CN * FS] = cn;
     }
   }
 
