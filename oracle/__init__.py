@@ -2,7 +2,7 @@
 
 ctypes binding of the plain fp64 C++ oracle.  Only tests/, __graft_entry__.smoke() and
 bench.py's cpu_baseline / --impl reference leg may import this package; the product
-(paper_1802_04449_b200) never does.
+(the CUDA package) never does.
 """
 from __future__ import annotations
 

@@ -147,8 +147,11 @@ __device__ __forceinline__ void limit_pi_P(R xi, R e, R P, R pi[10], unsigned& f
   }
 }
 
+#ifndef CLV_MINB
+#define CLV_MINB 2
+#endif
 template <typename R, bool VISC, int MODE>
-__global__ void __launch_bounds__(256, 2) stage_fused_kernel(const StageArgs<R> a) {
+__global__ void __launch_bounds__(256, CLV_MINB) stage_fused_kernel(const StageArgs<R> a) {
   constexpr bool USE_PI = VISC && (MODE != 0);
   constexpr int NF = VISC ? 14 : 4;                 // evolved fields of a buffer; extended slots follow
   constexpr int OX = NF * FS;                       // element offset of the extended slots inside an x-block
@@ -222,18 +225,25 @@ __global__ void __launch_bounds__(256, 2) stage_fused_kernel(const StageArgs<R> 
     }
     // pi fields: Q = u^tau pi, F_a = u^a pi   (Eq.29)
     if (USE_PI) {
-      int om = F_PI * FS;
+      // software-pipelined: the five loads of field m+1 are issued before the arithmetic of field m
+      R v[5];
+#pragma unroll
+      for (int p = 0; p < 5; ++p) v[p] = pp[p][F_PI * FS];
+      int om = (F_PI + 1) * FS;
 #pragma unroll 1
       for (int m = 0; m < 10; ++m, om += FS) {
+        R vn[5];
+        const int on = m < 9 ? om : F_PI * FS;      // last trip re-reads field 0 (L1 hit) instead of branching
+#pragma unroll
+        for (int p = 0; p < 5; ++p) vn[p] = pp[p][on];
         R q[5], f[5];
 #pragma unroll
-        for (int p = 0; p < 5; ++p) {
-          const R v = pp[p][om];
-          q[p] = g[p] * v; f[p] = ua[p] * v;
-        }
+        for (int p = 0; p < 5; ++p) { q[p] = g[p] * v[p]; f[p] = ua[p] * v[p]; }
         const R d = kt_div2(q, f, cl, cr, a.theta) * sc_pi;
         R* slot = &sS[m * 256 + tid];
         *slot = (ax == 0) ? -d : *slot - d;
+#pragma unroll
+        for (int p = 0; p < 5; ++p) v[p] = vn[p];
       }
     }
   }

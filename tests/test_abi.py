@@ -1,0 +1,65 @@
+"""-m "not gpu": the C-ABI library builds, loads without a GPU and exports every symbol include/*.h declares;
+argument validation and the no-CPU-fallback rule are checked without any compute call."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "clvisc_hydro.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(hydro_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported():
+    from paper_1802_04449_b200 import hydro
+    lib = hydro.load_library()
+    names = declared_symbols()
+    assert set(names) == set(hydro.SYMBOLS), (names, hydro.SYMBOLS)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_workspace_bytes_and_validation():
+    from paper_1802_04449_b200 import hydro
+    lib = hydro.load_library()
+    g = hydro.make_grid(301, 301, 201, 0.1, 0.1, 0.08)
+    w64, w32 = hydro.workspace_bytes(g, 64, 0.16), hydro.workspace_bytes(g, 32, 0.16)
+    # 3 buffers x 19 fields x (10 x-blocks of 32) x 301 x 201 cells x 8 B, plus gstar, tables, diag
+    cells_padded = 320 * 301 * 201
+    assert w64 >= 3 * 19 * cells_padded * 8 and w64 < 3.2 * 19 * cells_padded * 8
+    assert abs(w32 / w64 - 0.5) < 0.01
+    assert hydro.workspace_bytes(g, 64, 0.0) < w64 / 2          # ideal: 9 fields per buffer
+    assert hydro.workspace_bytes(hydro.make_grid(0, 4, 4, 1, 1, 1), 64, 0.0) == 0
+    assert hydro.workspace_bytes(g, 16, 0.0) == 0
+    assert lib.hydro_strerror(-2).decode().startswith("workspace")
+    # NULL arguments are rejected before any CUDA call
+    h = ctypes.c_void_p()
+    assert lib.hydro_create(ctypes.byref(h), None, 0.01, 0.4, None, 0.0, None) == -1
+    assert lib.hydro_step(None, 1) == -1 and lib.hydro_launch_count(None) == 0
+
+
+def test_no_cpu_fallback():
+    import torch
+    from paper_1802_04449_b200 import Hydro, HydroError, inputs
+    if torch.cuda.is_available():
+        pytest.skip("GPU present: covered by the gpu tests")
+    with pytest.raises(HydroError):
+        Hydro(4, 4, 4, 0.1, 0.1, 0.1, 0.01, 0.6, inputs.conformal_eos(), 0.0)
+
+
+def test_product_never_imports_oracle():
+    pkg = os.path.join(ROOT, "paper_1802_04449_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "clvisc_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_1802_04449_b200" not in txt and "libclvisc_hydro" not in txt, f
