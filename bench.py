@@ -61,16 +61,17 @@ class ClockSampler(threading.Thread):
                 out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
                                       "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
                 if out.returncode == 0 and out.stdout.strip():
-                    self.rows.append([c.strip() for c in out.stdout.strip().split(",")])
+                    self.rows.append([time.perf_counter()] + [c.strip() for c in out.stdout.strip().split(",")])
             except Exception:
                 pass
             self._stop_evt.wait(0.2)
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
         self._stop_evt.set()
         self.join(timeout=10)
         sm, reasons, mx = [], set(), None
-        for r in self.rows:
+        inside = [r[1:] for r in self.rows if t0 is not None and t0 <= r[0] <= t1]
+        for r in (inside or [r[1:] for r in self.rows]):
             try:
                 sm.append(float(r[0])); mx = float(r[1])
             except Exception:
@@ -79,7 +80,7 @@ class ClockSampler(threading.Thread):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "samples": len(sm), "samples_inside_timed_region": len(inside)}
 
 
 def sub_config(nx, ny, nz, partons):
@@ -130,7 +131,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--precision", type=int, default=64, choices=(64, 32))
     ap.add_argument("--kernel", type=int, default=0)
@@ -145,7 +146,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1802_04449_b200 import from_config
+    from paper_1802_04449_b200 import from_config, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -162,7 +163,7 @@ def main():
     if (nx, ny, nz) != (301, 301, 201):
         cfg.extra["partons"] = max(8, int(round(8000 * cfg.cells / (301.0 * 301 * 201))))
     eos = inputs.crossover_table()
-    T, _ = inputs.ic_partons(cfg, inputs.seed_for(4, variant=rank))     # one seeded event per rank
+    T, _ = inputs.ic_partons(cfg, replicas.rank_seed(4, rank))     # one seeded event per rank
     npdt = np.float64 if args.precision == 64 else np.float32
     tdt = torch.float64 if args.precision == 64 else torch.float32
 
@@ -178,12 +179,13 @@ def main():
             torch.cuda.synchronize(dev)
 
     # ---- device-resident timing ----------------------------------------------------------------
-    h.step(args.warmup)
-    barrier()
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start()
+    h.step(args.warmup)
+    barrier()
     l0 = h.launch_count()
+    tw0 = time.perf_counter()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record(stream)
     h.step(args.steps)
@@ -191,14 +193,10 @@ def main():
     barrier()
     ms = ev0.elapsed_time(ev1)
     launches = h.launch_count() - l0
-    clocks = sampler.stop() if sampler else None
+    clocks = sampler.stop(tw0, time.perf_counter()) if sampler else None
     d = h.diag()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    value, ms = replicas.aggregate_rate(cfg.cells, args.steps, ms, world, dev)
     ms_per_step = ms / args.steps
-    value = world * cfg.cells * args.steps / (ms * 1e-3)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): load -> step -> read, every step ------
     N = cfg.cells
@@ -220,10 +218,7 @@ def main():
         e2e_step()
     barrier()
     e2e_s = max(time.perf_counter() - t0, 1e-9)
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, dev)
     esz = 8 if args.precision == 64 else 4
     e2e = {"value": world * N * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz,
            "d2h_bytes_per_step": 15 * N * esz, "steps": args.e2e_steps,
@@ -244,7 +239,13 @@ def main():
     if os.path.exists(tp):
         with open(tp) as f:
             traffic = json.load(f).get(f"f{args.precision}_k{h_kernel_name(args.kernel)}")
+    # second view: the same launch against the plain fp64 (fp32) pipe, 3 400 arithmetic
+    # instructions per cell per stage on 148 SMs x 64 (128) lanes at the SM clock sampled during the run
+    lanes = 64 if args.precision == 64 else 128
+    sm_hz = 1e6 * ((clocks or {}).get("sm_mhz") or 1965.0)
+    alu_frac = (3400.0 * cfg.cells / avg_launch_s) / (148 * lanes * sm_hz)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "alu_frac": alu_frac,
                 "traffic": traffic, "peak_source": peak_src, "kernel": "fused RK2 stage kernel (avg of stage 1 and 2)",
                 "algorithmic_bytes_per_launch": algo_per_launch, "avg_launch_ms": avg_launch_s * 1e3}
 
