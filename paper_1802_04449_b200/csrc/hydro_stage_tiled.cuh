@@ -55,9 +55,10 @@ __device__ __forceinline__ R kt_div2(const R q[5], const R f[5], R cl, R cr, R t
   const R df0 = f[1] - f[0], df1 = f[2] - f[1], df2 = f[3] - f[2], df3 = f[4] - f[3];
   const R hq1 = hmm(dq0, dq1, theta), hq2 = hmm(dq1, dq2, theta), hq3 = hmm(dq2, dq3, theta);
   const R hf1 = hmm(df0, df1, theta), hf2 = hmm(df1, df2, theta), hf3 = hmm(df2, df3, theta);
-  const R Hr = ((f[3] - hf3) + (f[2] + hf2)) - cr * ((q[3] - hq3) - (q[2] + hq2));
-  const R Hl = ((f[2] - hf2) + (f[1] + hf1)) - cl * ((q[2] - hq2) - (q[1] + hq1));
-  return Hr - Hl;
+  // Hr - Hl with the f-part collected: (f3 + f2 - hf3 + hf2) - (f2 + f1 - hf2 + hf1) = (df1 + df2) - hf3 - hf1 + 2 hf2
+  const R fpart = ((df1 + df2) - (hf3 + hf1)) + R(2) * hf2;
+  const R qr = (dq2 - hq3) - hq2, ql = (dq1 - hq2) - hq1;
+  return fpart - cr * qr + cl * ql;
 }
 
 // signal speeds of one cell along the three axes from u~ (A6); cs2 from the EoS at the cell
@@ -97,6 +98,7 @@ __device__ __forceinline__ void rootfind_warp(const EosDev<R>& eos, R M0, R Mx, 
     P = e * R(1.0 / 3.0); cs2 = R(1.0 / 3.0);
   } else {
     const R tol = (sizeof(R) == 8) ? R(1e-15) : R(2e-7);
+    const R tol2 = (sizeof(R) == 8) ? R(1e-9) : R(1e-4);
     R lo = R(0), hi = M0;
     e = e_start;
     if (!(e > lo && e < hi)) e = M0 - M2 / (M0 + M0 * R(1.0 / 3.0));
@@ -112,6 +114,9 @@ __device__ __forceinline__ void rootfind_warp(const EosDev<R>& eos, R M0, R Mx, 
       R en = e - g / dg;
       if (!(en >= lo && en <= hi)) en = R(0.5) * (lo + hi);
       e = conv ? e : en;
+      // Newton converges quadratically on the (piecewise linear, convex) g: a step taken from a residual
+      // below sqrt(tol) lands below tol, so the warp can leave without another evaluation
+      if (__all_sync(0xffffffffu, !(abs_(g) > tol2 * M0))) break;
     }
     eos_P(eos, e, P, cs2);
     const R g = M0 - M2 / (M0 + P) - e;
