@@ -38,7 +38,9 @@ __device__ __forceinline__ double hmm(double dm, double dp, double theta) {
   const double h = fabs(dm + dp) * 0.5;
   const double m = t < h ? t : h;
   const int hm = __double2hiint(dm), hp = __double2hiint(dp);
-  const int khi = ((hm ^ hp) >= 0) ? (0x3fe00000 | (hm & 0x80000000)) : 0;     // +-0.5 or 0
+  int k;                                                      // high word of copysign(0.5, dm), one LOP3
+  asm("lop3.b32 %0, %1, 0x80000000, %2, 0xEA;" : "=r"(k) : "r"(hm), "r"(0x3fe00000));     // (a & b) | c
+  const int khi = ((hm ^ hp) >= 0) ? k : 0;                   // +-0.5 or 0
   return m * __hiloint2double(khi, 0);
 }
 __device__ __forceinline__ float hmm(float dm, float dp, float theta) {
