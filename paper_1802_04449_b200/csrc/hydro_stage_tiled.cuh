@@ -235,25 +235,27 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
     }
     // pi fields: Q = u^tau pi, F_a = u^a pi   (Eq.29)
     if (USE_PI) {
-      // software-pipelined: the five loads of field m+1 are issued before the arithmetic of field m
-      R v[5];
+      // two fields per trip: their 12 minmod chains interleave (ILP for the 4 warps per scheduler), the field
+      // offsets inside a trip are immediates and the five star pointers are bumped once per trip
+      const R* __restrict__ pq[5];
 #pragma unroll
-      for (int p = 0; p < 5; ++p) v[p] = pp[p][F_PI * FS];
-      int om = (F_PI + 1) * FS;
+      for (int p = 0; p < 5; ++p) pq[p] = pp[p] + F_PI * FS;
+      R* slot = &sS[tid];
 #pragma unroll 1
-      for (int m = 0; m < 10; ++m, om += FS) {
-        R vn[5];
-        const int on = m < 9 ? om : F_PI * FS;      // last trip re-reads field 0 (L1 hit) instead of branching
+      for (int t = 0; t < 5; ++t) {
+        R qa[5], fa[5], qb[5], fb[5];
 #pragma unroll
-        for (int p = 0; p < 5; ++p) vn[p] = pp[p][on];
-        R q[5], f[5];
-#pragma unroll
-        for (int p = 0; p < 5; ++p) { q[p] = g[p] * v[p]; f[p] = ua[p] * v[p]; }
-        const R d = kt_div2(q, f, cl, cr, a.theta) * sc_pi;
-        R* slot = &sS[m * 256 + tid];
-        *slot = (ax == 0) ? -d : *slot - d;
-#pragma unroll
-        for (int p = 0; p < 5; ++p) v[p] = vn[p];
+        for (int p = 0; p < 5; ++p) {
+          const R va = pq[p][0], vb = pq[p][FS];
+          qa[p] = g[p] * va; fa[p] = ua[p] * va;
+          qb[p] = g[p] * vb; fb[p] = ua[p] * vb;
+          pq[p] += 2 * FS;
+        }
+        const R da = kt_div2(qa, fa, cl, cr, a.theta) * sc_pi;
+        const R db = kt_div2(qb, fb, cl, cr, a.theta) * sc_pi;
+        slot[0] = (ax == 0) ? -da : slot[0] - da;
+        slot[256] = (ax == 0) ? -db : slot[256] - db;
+        slot += 2 * 256;
       }
     }
   }
