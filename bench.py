@@ -139,6 +139,8 @@ def main():
     ap.add_argument("--grid", default="301,301,201", help="nx,ny,nz (default = configs[4])")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--eta-over-s", type=float, default=0.16,
+                    help="context runs only (0 = the ideal-fluid path, PAPER.md Table II); the headline is 0.16")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -159,7 +161,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     nx, ny, nz = [int(v) for v in args.grid.split(",")]
-    cfg = inputs.config4(nx=nx, ny=ny, nz=nz)
+    cfg = inputs.config4(nx=nx, ny=ny, nz=nz, eta_over_s=args.eta_over_s)
     if (nx, ny, nz) != (301, 301, 201):
         cfg.extra["partons"] = max(8, int(round(8000 * cfg.cells / (301.0 * 301 * 201))))
     eos = inputs.crossover_table()
@@ -230,7 +232,8 @@ def main():
 
     # ---- roofline of the dominant kernel (the fused stage kernel: 2 launches per step) ------------------
     peak, peak_src = measured_hbm_peak()
-    algo_per_launch = ALGO_BYTES_PER_CELL_STEP[args.precision] * cfg.cells / 2.0
+    words = 73 if args.eta_over_s > 0 else 20            # compulsory words per cell per RK2 step
+    algo_per_launch = words * (args.precision // 8) * cfg.cells / 2.0
     avg_launch_s = ms * 1e-3 / launches
     achieved = algo_per_launch / avg_launch_s / 1e9
     traffic = None
@@ -257,7 +260,7 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
             "config": {"workload": f"configs[4]: {nx}x{ny}x{nz} cells, dx=dy=0.1 fm, deta=0.08, tau0=0.4, dtau=0.01, "
-                                   f"eta/s=0.16, crossover EoS table (2000 nodes), {cfg.extra['partons']} seeded "
+                                   f"eta/s={args.eta_over_s:g}, crossover EoS table (2000 nodes), {cfg.extra['partons']} seeded "
                                    "partons with momentum, outflow boundaries",
                        "cells": cfg.cells, "precision": args.precision, "kernel": args.kernel,
                        "l2": "working set (3 x 14 fields) >> 126 MB L2, no flush needed",
