@@ -277,7 +277,7 @@ def main():
 
 
 def h_kernel_name(k):
-    return {0: "default", 1: "ref", 2: "tiled"}.get(k, str(k))
+    return {0: "default", 1: "ref", 2: "fused"}.get(k, str(k))
 
 
 if __name__ == "__main__":

@@ -23,8 +23,8 @@
  *   - the caller owns every buffer it passes, including the workspace; the library never frees
  *     them and keeps no pointer to field arguments after the call returns.  The workspace must
  *     stay alive (and untouched) until hydro_destroy.
- *   - return value: 0 success; negative = error (below); positive (hydro_step, hydro_diag) = warning
- *     bit mask.  No exceptions, no global state; a context is not thread-safe.
+ *   - return value: 0 success; negative = error (below); hydro_diag returns a non-negative warning bit mask
+ *     (hydro_step never synchronises, so warnings are reported by hydro_diag only).  No exceptions, no global state; a context is not thread-safe.
  *   - the whole path runs in CUDA kernels for sm_100a; there is no CPU fallback: without a usable
  *     device every compute entry point returns HYDRO_ECUDA.
  */
@@ -72,7 +72,8 @@ typedef struct {
  * <= 0 selects the default 0.999 (gamma <= 22.4; A7 gives the evidence); root_iters: fixed Newton iteration
  * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
  * stream); workspace: DEVICE memory of at least hydro_workspace_bytes(), 256-byte aligned.
- * kernel: 0 = default (fastest validated), 1 = reference per-cell kernel, 2 = tiled kernel. */
+ * kernel: 0 = default (= 2), 1 = reference kernel (re-derives P, u^tau, c_a at every stencil point),
+ * 2 = fused kernel on the extended state (hydro_stage_fused.cuh). */
 typedef struct {
   int precision;
   double minmod_theta, e_floor, pi_limit_xi, v_max;

@@ -21,7 +21,7 @@
 #include <vector>
 
 #include "hydro_stage_ref.cuh"
-#include "hydro_stage_tiled.cuh"
+#include "hydro_stage_fused.cuh"
 
 namespace clv {
 
@@ -246,7 +246,7 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
 template <typename R, bool VISC, int MODE>
 int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
   if (c->kernel == 2) {
-    launch_stage_tiled<R, VISC, MODE>(a, c->stream);
+    launch_stage_fused<R, VISC, MODE>(a, c->stream);
   } else {
     dim3 block(32, 8, 1);
     dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, a.nz);

@@ -1,7 +1,7 @@
-// hydro_stage_tiled.cuh -- "kernel 2": the production stage kernel.
+// hydro_stage_fused.cuh -- "kernel 2": the production stage kernel (fused stage on the extended state).
 //
 // Same fused stage as hydro_stage_ref.cuh (one launch per RK2 stage, one thread per cell), re-organised
-// around what the ncu profile of kernel 1 showed (profiles/round1_v1_ref_kernel.md: fp64 pipe 30 %,
+// around what the ncu profile of kernel 1 showed (profiles/round1_kernel1.md: fp64 pipe 30 %,
 // 15 k instructions per cell, 255 registers, 12 % occupancy):
 //   * EXTENDED STATE: the producing kernel appends P, u^tau and the three signal speeds c_x, c_y, c_eta
 //     of every cell to the state it writes (5 extra words), so the 13-point star is READ, never
@@ -423,7 +423,7 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
 }
 
 template <typename R, bool VISC, int MODE>
-void launch_stage_tiled(const StageArgs<R>& a, cudaStream_t stream) {
+void launch_stage_fused(const StageArgs<R>& a, cudaStream_t stream) {
   dim3 block(32, 8, 1);
   dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, a.nz);
   stage_fused_kernel<R, VISC, MODE><<<grid, block, 0, stream>>>(a);

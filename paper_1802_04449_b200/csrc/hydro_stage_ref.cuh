@@ -2,7 +2,7 @@
 // memory through L1/L2.  Every step of the RK2 stage is fused in this one kernel (KT fluxes on three
 // axes for 4 + 10 fields, geometric source, velocity gradients, Israel-Stewart source, stage update,
 // root-find, pi limiter, CFL / e_max reductions): one launch per stage.  It is the simple, obviously
-// structured CUDA statement of the method; the tiled kernel (hydro_stage_tiled.cuh) must agree with it.
+// structured CUDA statement of the method; the fused extended-state kernel (hydro_stage_fused.cuh) must agree with it.
 //
 // Stages (Eq.49-54; A10-A12, A26):
 //   MODE 1: RHS on state n at tau_n, time derivative from u* = 2u^n - u^{n-1}; writes state ' and u*^tau.
