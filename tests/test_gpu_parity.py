@@ -172,3 +172,27 @@ def test_errors_are_loud(conformal):
     h = Hydro(4, 4, 4, 0.1, 0.1, 0.1, 0.01, 0.6, conformal, 0.0)
     with pytest.raises(HydroError):
         h.step(1)      # before load
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("shape,bc", [((64, 16, 3), (1, 0, 1)), ((32, 8, 1), (1, 1, 0)), ((5, 3, 2), (0, 1, 1)),
+                                      ((97, 2, 6), (1, 1, 1))])
+def test_tile_exact_and_tiny_grids(crossover, kernel, shape, bc):
+    # grids that are an exact multiple of the 32x8 thread tile (periodic wrap across x-blocks), a single tile,
+    # grids smaller than the 2-cell stencil reach in some axis, and a 4-block row with a ragged 1-cell tail
+    nx, ny, nz = shape
+    e, v, pi = inputs.ic_random_smooth(nx, ny, nz, seed=31, vmax=0.45)
+    from parity_util import pressure
+    P = pressure(crossover, e)
+    g2 = 1.0 / (1.0 - (v ** 2).sum(0))
+    T = np.stack([(e + P) * g2 - P, (e + P) * g2 * v[0], (e + P) * g2 * v[1], (e + P) * g2 * v[2]]) + pi[:4]
+    cfg = inputs.Config("t", nx, ny, nz, 0.2, 0.25, 0.3, 0.8, 0.02, 3, 0.1, "crossover", bc=bc)
+    o, g = run_pair(cfg, crossover, T, pi, 0, gkw=dict(kernel=kernel))
+    o.step(3); g.step(3)
+    er = errors(crossover, o.read(), g.read())
+    print("grid", shape, bc, er)
+    assert er["rel_e"] <= 1e-10 and er["rel_T"] <= 1e-10 and er["rel_pi"] <= 1e-10
+    o32, g32 = run_pair(cfg, crossover, T, pi, 0, gkw=dict(kernel=kernel, precision=32))
+    o32.step(3); g32.step(3)
+    er = errors(crossover, o32.read(), g32.read())
+    assert er["l2_e"] <= 2e-4 and er["l2_T"] <= 2e-4 and er["rel_e"] < 1e-3
