@@ -148,6 +148,10 @@ __device__ __forceinline__ void is_source(const R ut[4], const R grad[4][4], con
   const R inv_taupi = T * inv_5etas_hbarc;      // 1/tau_pi = T s/(5 eta_v)
   const R eta_over_taupi = (e + P) * R(0.2);    // eta_v/tau_pi = (e+P)/5
   const int IDX[4][4] = {{0, 1, 2, 3}, {1, 4, 5, 6}, {2, 5, 7, 8}, {3, 6, 8, 9}};
+  R w[4];
+#pragma unroll
+  for (int n = 0; n < 4; ++n)
+    w[n] = pi[IDX[n][0]] * Du[0] - pi[IDX[n][1]] * Du[1] - pi[IDX[n][2]] * Du[2] - pi[IDX[n][3]] * Du[3];
 #pragma unroll
   for (int m = 0; m < 4; ++m)
 #pragma unroll
@@ -157,11 +161,8 @@ __device__ __forceinline__ void is_source(const R ut[4], const R grad[4][4], con
                     R(2.0 / 3.0) * ((m == n ? gm[m] : R(0)) - ut[m] * ut[n]) * theta_exp;
       const R p = pi[IDX[m][n]];
       R src = eta_over_taupi * sig - p * inv_taupi - p * theta_exp * R(1.0 / 3.0);
-      R contr = R(0);
-#pragma unroll
-      for (int b = 0; b < 4; ++b)
-        contr += (ut[m] * pi[IDX[n][b]] + ut[n] * pi[IDX[m][b]]) * (gm[b] * Du[b]);
-      src -= contr;
+      // (u^m pi^{n b} + u^n pi^{m b}) g_{b a} Du^a with w^n = pi^{n b} g_{b a} Du^a formed once per row
+      src -= ut[m] * w[n] + ut[n] * w[m];
       if (milne) {
         R I = R(0);   // Eq.35-38 in the general form (A2)
         if (m == 0) I += pi[IDX[3][n]];
