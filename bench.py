@@ -252,7 +252,7 @@ def main():
                 "algorithmic_bytes_per_launch": algo_per_launch, "avg_launch_ms": avg_launch_s * 1e3}
 
     cpu = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:      # rank 0 at N = 1 only
         rate, threads, sample, _ = cpu_oracle_rate(96, 96, 64, 2)
         cpu = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
 
