@@ -52,6 +52,29 @@ def test_no_cpu_fallback():
         Hydro(4, 4, 4, 0.1, 0.1, 0.1, 0.01, 0.6, inputs.conformal_eos(), 0.0)
 
 
+def test_c_abi_create_without_device_returns_ecuda():
+    # straight through the C ABI, no torch involved: valid arguments, a (never dereferenced) aligned workspace
+    # pointer, but no CUDA device -> HYDRO_ECUDA (-3) and no context
+    import torch
+    from ctypes import byref, c_double, c_void_p, POINTER
+    from paper_1802_04449_b200 import hydro
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    lib = hydro.load_library()
+    g = hydro.make_grid(8, 8, 8, 0.1, 0.1, 0.1)
+    e = hydro.hydro_eos(); e.kind, e.n, e.e_min, e.e_max, e.c_sb = 0, 0, 0.0, 0.0, 15.6
+    o = hydro.hydro_opts()
+    o.precision, o.minmod_theta, o.e_floor, o.pi_limit_xi, o.v_max = 64, 1.1, 1e-7, 1.0, 0.0
+    o.workspace, o.workspace_bytes = c_void_p(1 << 20), hydro.workspace_bytes(g, 64, 0.1)
+    h = c_void_p()
+    assert lib.hydro_create(byref(h), byref(g), 0.01, 0.6, byref(e), 0.1, byref(o)) == -3
+    assert not h.value
+    o.workspace_bytes = 16                                       # too small is reported before the device check
+    assert lib.hydro_create(byref(h), byref(g), 0.01, 0.6, byref(e), 0.1, byref(o)) == -2
+    o.minmod_theta = 2.5
+    assert lib.hydro_create(byref(h), byref(g), 0.01, 0.6, byref(e), 0.1, byref(o)) == -1
+
+
 def test_product_never_imports_oracle():
     pkg = os.path.join(ROOT, "paper_1802_04449_b200")
     for dirpath, _, files in os.walk(pkg):
