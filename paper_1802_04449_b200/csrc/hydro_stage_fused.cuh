@@ -158,7 +158,8 @@ __device__ __forceinline__ void limit_pi_P(R xi, R e, R P, R pi[10], unsigned& f
 #define CLV_MINB 2
 #endif
 #ifndef CLV_MINB32
-#define CLV_MINB32 3     // fp32: 80 registers, 24 warps per SM (measured 10 % faster than 2 blocks)
+#define CLV_MINB32 2     // fp32 blocks per SM; with the unrolled axis loop 2 (128 registers, no spills) measured 9.25 ms
+                         // per step against 9.9 (3 blocks, 80 registers) and 9.5 (4 blocks, 64 registers)
 #endif
 template <typename R, bool VISC, int MODE>
 __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB)) stage_fused_kernel(const StageArgs<R> a) {
