@@ -51,6 +51,10 @@ def _load():
         lib.oracle_rhs.argtypes = [ctypes.c_void_p, dp, ctypes.c_double, dp, dp]
         lib.oracle_eos.argtypes = [ctypes.c_void_p, ctypes.c_double, dp]
         lib.oracle_rootfind.argtypes = [ctypes.c_void_p, dp, dp]
+        lib.oracle_limit_pi.restype = ctypes.c_int
+        lib.oracle_limit_pi.argtypes = [ctypes.c_void_p, ctypes.c_double, dp]
+        lib.oracle_set_option.restype = ctypes.c_int
+        lib.oracle_set_option.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double]
         _lib = lib
     return _lib
 
@@ -143,6 +147,18 @@ class Oracle:
         out = np.zeros(3)
         _load().oracle_eos(self._h, float(e), _p(out))
         return tuple(out)
+
+    def limit_pi(self, e, pi10):
+        """pi limiter (A14) on one cell: returns (scaled pi[10], acted?)."""
+        p = np.array(pi10, dtype=np.float64)
+        acted = _load().oracle_limit_pi(self._h, float(e), _p(p))
+        return p, bool(acted)
+
+    OPT_HEUN_PRINTED = 0
+
+    def set_option(self, key, value):
+        if _load().oracle_set_option(self._h, int(key), float(value)):
+            raise ValueError("oracle_set_option: unknown key")
 
     def rootfind(self, M4):
         M4 = np.ascontiguousarray(M4, dtype=np.float64)

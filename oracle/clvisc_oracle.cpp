@@ -9,10 +9,14 @@
 //   * KT central scheme                       PAPER.md:193-213  (Eq.40-44)
 //   * RK2 predictor/corrector with u* = 2u^n - u^{n-1}   PAPER.md:225-239 (Eq.49-54)
 //   * root-find T_ideal = T - pi -> e, u      PAPER.md:229,235  (Eq.51,54)
-// Pins (tests/test_oracle_*.py): ideal + Israel-Stewart Bjorken, Gubser (ideal closed form and
-// IS ODE), exact conservation, brute-force per-cell evaluator on 4^3, root-find closed form,
-// EoS closed form, mirror symmetry.  Unpinned conventions (shared rule, not shared code):
-// A8 dynamic floor, A14 pi limiter, A23 bootstrap of u^{-1} -- "parity unpinned" for those.
+// Pins (tests/test_oracle_*.py): ideal + Israel-Stewart Bjorken, Gubser (ideal closed form and IS ODE, to tau = 4
+// against the survey's independent probe numbers), exact conservation, brute-force per-cell evaluator on 4^3,
+// root-find closed form, EoS closed form, mirror symmetry, Riemann fan; the Milne terms that need u~^eta != 0
+// (Eq.24-26, 31, 35-38) by a Minkowski-static fluid, a slice-uniform shear tensor and the Poincare-shifted Gubser
+// PDE residual (test_oracle_milne_pins.py); the pi limiter (A14) by its invariant, the bootstrap of u^{-1} (A23)
+// against ideal Gubser at O(h^2), strict Eq.53 (A12) and the printed Heun form (A26) by convergence / difference
+// (test_oracle_limiter_bootstrap.py).  Still a shared convention without an external pin: the value of the
+// dynamic floor (A8) -- "parity unpinned" for that one rule.
 //
 // Notation: tilde/tetrad components, g~ = diag(1,-1,-1,-1); u~ = gamma(1,vx,vy,veta);
 // frame tensor T_f^{mu nu} = (e+P)u~^mu u~^nu - P g~^{mu nu} + pi~^{mu nu};  paper's T~ = tau*T_f.
@@ -92,6 +96,7 @@ struct Oracle {
   double dtau, tau0, eta_s;
   double theta = 1.1, e_floor = 1e-7, xi = 1.0, v_max = 1.0 - 1e-10;
   int strict_eq53 = 0;
+  int heun_printed = 0;   // A26: 0 = Shu-Osher bookkeeping (default), 1 = Eq.52-53 exactly as printed
   int step = 0;
   bool loaded = false;
   size_t N;
@@ -363,6 +368,7 @@ void bootstrap_history(Oracle& o) {
   rhs(o, s, false, nullptr, o.tau0, ST, SP, nullptr);
   double tf0 = milne ? o.tau0 : 1.0, tf1 = milne ? o.tau0 + o.dtau : 1.0;
   long dummy1 = 0, dummy2 = 0;
+#pragma omp parallel for reduction(+ : dummy1, dummy2)
   for (size_t c = 0; c < N; ++c) {
     double QT[4], M[4], e1, u1[3];
     conserved_T(o, s, c, false, tf0, QT);
@@ -384,6 +390,7 @@ void step_once(Oracle& o) {
   // ---- stage 1 at tau_n -------------------------------------------------------------------
   std::vector<double> dtu[4], gstar(N);
   for (int m = 0; m < 4; ++m) dtu[m].resize(N);
+#pragma omp parallel for
   for (size_t c = 0; c < N; ++c) {
     double us[3], g2 = 1.0, gs2 = 1.0;
     for (int a = 0; a < 3; ++a) {
@@ -403,6 +410,8 @@ void step_once(Oracle& o) {
   for (int a = 0; a < 3; ++a) u1[a].resize(N);
   for (int m = 0; m < 10; ++m) pi1[m].assign(N, 0.0);
   for (int m = 0; m < 4; ++m) QTn[m].resize(N);
+  long nfl = 0, ncl = 0, nli = 0;   // event counters of this step (summed over the flat cell loops)
+#pragma omp parallel for reduction(+ : nfl, ncl, nli)
   for (size_t c = 0; c < N; ++c) {
     double QT[4], pp[10] = {0}, M[4], uu[3];
     conserved_T(o, sn, c, visc, tf_n, QT);
@@ -412,13 +421,14 @@ void step_once(Oracle& o) {
       for (int m = 0; m < 10; ++m) pp[m] = (gn * o.pi[m][c] + h * SP[m][c]) / gstar[c];   // Eq.49
     }
     for (int m = 0; m < 4; ++m) M[m] = (QT[m] + h * ST[m][c]) / tf_1 - pp[m];              // Eq.50-51
-    rootfind(o, M, &e1[c], uu, &o.n_floor, &o.n_clamp);
-    if (visc) limit_pi(o, e1[c], pp, &o.n_limit);
+    rootfind(o, M, &e1[c], uu, &nfl, &ncl);
+    if (visc) limit_pi(o, e1[c], pp, &nli);
     for (int a = 0; a < 3; ++a) u1[a][c] = uu[a];
     for (int m = 0; m < 10; ++m) pi1[m][c] = pp[m];
   }
 
   // ---- stage 2 at tau_{n+1} ---------------------------------------------------------------
+#pragma omp parallel for
   for (size_t c = 0; c < N; ++c) {
     double g2 = 1.0, g12 = 1.0;
     for (int a = 0; a < 3; ++a) { g2 += o.u[a][c] * o.u[a][c]; g12 += u1[a][c] * u1[a][c]; }
@@ -429,16 +439,23 @@ void step_once(Oracle& o) {
   std::vector<double> ST1[4], SP1[10];
   rhs(o, s1, visc, dtu, tau_1, ST1, SP1, nullptr);
 
-  // Heun in Shu-Osher form (A26): Q^{n+1} = 1/2 [Q^n + Q(state') + h S_tot(state')], where
+  // Heun in Shu-Osher form (A26, default): Q^{n+1} = 1/2 [Q^n + Q(state') + h S_tot(state')], where
   // Q(state') is rebuilt from the stored stage-1 state (after floor / clamp / limiter).
+  // heun_printed = 1: Eq.52-53 exactly as printed, Q^{n+1} = Q^n + h/2 (S_tot(n) + S_tot(')); the two agree to
+  // rounding unless the floor, the v_max clamp or the pi limiter acted in stage 1.
   std::vector<double> pinew[10];
   for (int m = 0; m < 10; ++m) pinew[m].assign(N, 0.0);
   if (visc) {
+#pragma omp parallel for
     for (size_t c = 0; c < N; ++c) {
       double gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
       double g1 = std::sqrt(1.0 + u1[0][c] * u1[0][c] + u1[1][c] * u1[1][c] + u1[2][c] * u1[2][c]);
-      for (int m = 0; m < 10; ++m)
-        pinew[m][c] = 0.5 * (gn * o.pi[m][c] + gstar[c] * pi1[m][c] + h * SP1[m][c]) / g1;   // Eq.52
+      for (int m = 0; m < 10; ++m) {
+        if (o.heun_printed)
+          pinew[m][c] = (gn * o.pi[m][c] + 0.5 * h * (SP[m][c] + SP1[m][c])) / g1;             // Eq.52 as printed
+        else
+          pinew[m][c] = 0.5 * (gn * o.pi[m][c] + gstar[c] * pi1[m][c] + h * SP1[m][c]) / g1;   // Eq.52
+      }
     }
     if (o.strict_eq53) {   // Eq.53 as printed: stage-2 T source evaluated with pi^{n+1} (A12)
       State s1b = view(e1, u1, pinew, true);
@@ -446,18 +463,24 @@ void step_once(Oracle& o) {
       rhs(o, s1b, true, dtu, tau_1, ST1, SPdummy, nullptr);
     }
   }
+#pragma omp parallel for reduction(+ : nfl, ncl, nli)
   for (size_t c = 0; c < N; ++c) {
     double QT1[4], M[4], pp[10], en, uu[3];
     conserved_T(o, s1, c, visc, tf_1, QT1);
     for (int m = 0; m < 10; ++m) pp[m] = pinew[m][c];
-    for (int m = 0; m < 4; ++m)
-      M[m] = 0.5 * (QTn[m][c] + QT1[m] + h * ST1[m][c]) / tf_1 - pp[m];                      // Eq.53-54
-    rootfind(o, M, &en, uu, &o.n_floor, &o.n_clamp);
-    if (visc) limit_pi(o, en, pp, &o.n_limit);
+    for (int m = 0; m < 4; ++m) {
+      if (o.heun_printed)
+        M[m] = (QTn[m][c] + 0.5 * h * (ST[m][c] + ST1[m][c])) / tf_1 - pp[m];                // Eq.53-54 as printed
+      else
+        M[m] = 0.5 * (QTn[m][c] + QT1[m] + h * ST1[m][c]) / tf_1 - pp[m];                    // Eq.53-54
+    }
+    rootfind(o, M, &en, uu, &nfl, &ncl);
+    if (visc) limit_pi(o, en, pp, &nli);
     for (int a = 0; a < 3; ++a) { o.uprev[a][c] = o.u[a][c]; o.u[a][c] = uu[a]; }
     o.e[c] = en;
     for (int m = 0; m < 10; ++m) o.pi[m][c] = pp[m];
   }
+  o.n_floor += nfl; o.n_clamp += ncl; o.n_limit += nli;
   o.e_max_seen = *std::max_element(o.e.begin(), o.e.end());
   o.step += 1;
 }
@@ -498,13 +521,16 @@ void oracle_destroy(void* h) { delete static_cast<Oracle*>(h); }
 int oracle_load(void* h, const double* T, const double* pi) {
   Oracle& o = *static_cast<Oracle*>(h);
   const size_t N = o.N;
+  long nfl = 0, ncl = 0;
+#pragma omp parallel for reduction(+ : nfl, ncl)
   for (size_t c = 0; c < N; ++c) {
     double M[4], uu[3];
     for (int m = 0; m < 10; ++m) o.pi[m][c] = (pi && o.viscous()) ? pi[m * N + c] : 0.0;
     for (int m = 0; m < 4; ++m) M[m] = T[m * N + c] - o.pi[m][c];
-    rootfind(o, M, &o.e[c], uu, &o.n_floor, &o.n_clamp);
+    rootfind(o, M, &o.e[c], uu, &nfl, &ncl);
     for (int a = 0; a < 3; ++a) o.u[a][c] = uu[a];
   }
+  o.n_floor += nfl; o.n_clamp += ncl;
   o.step = 0;
   bootstrap_history(o);
   o.e_max_seen = *std::max_element(o.e.begin(), o.e.end());
@@ -600,6 +626,22 @@ int oracle_set_state(void* h, const double* e, const double* u, const double* pi
 void oracle_eos(void* h, double e, double* out3) {
   Oracle& o = *static_cast<Oracle*>(h);
   eos_eval(o.eos, e, &out3[0], &out3[1], &out3[2]);
+}
+
+// Test hook: the pi limiter (A14) on one cell; pi10 is scaled in place, returns 1 when it acted.
+int oracle_limit_pi(void* h, double e, double* pi10) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  long n = 0;
+  limit_pi(o, e, pi10, &n);
+  return int(n);
+}
+
+// Options that are not part of oracle_create's argument list.  key 0: heun_printed (A26; 0 default, 1 = Eq.52-53
+// as printed).  Returns 0, or -1 for an unknown key.
+int oracle_set_option(void* h, int key, double value) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (key == 0) { o.heun_printed = value != 0.0 ? 1 : 0; return 0; }
+  return -1;
 }
 
 void oracle_rootfind(void* h, const double* M4, double* out4) {

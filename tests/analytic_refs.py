@@ -103,3 +103,40 @@ class Gubser:
         P = e / 3.0
         T = np.stack([(e + P) * u[0] * u[m] - (P if m == 0 else 0.0) + pi[m] for m in range(4)])
         return T, pi
+
+
+def boost_tilde(u, pi, delta):
+    """Re-express tilde components given in a Milne tetrad at rapidity eta' in the tetrad at eta = eta' - delta:
+    a (tau, eta)-block boost by delta on every index (Eq.18-23 define the tetrad).
+    u: [4,...] (tau, x, y, eta); pi: [10,...] in the order tt, tx, ty, tn, xx, xy, xn, yy, yn, nn."""
+    ch, sh = np.cosh(delta), np.sinh(delta)
+    shape = u.shape[1:]
+    L = np.zeros((4, 4) + shape)
+    L[0, 0] = ch; L[0, 3] = sh; L[3, 0] = sh; L[3, 3] = ch
+    L[1, 1] = 1.0; L[2, 2] = 1.0
+    un = np.einsum("ab...,b...->a...", L, u)
+    idx = [(0, 0), (0, 1), (0, 2), (0, 3), (1, 1), (1, 2), (1, 3), (2, 2), (2, 3), (3, 3)]
+    P = np.zeros((4, 4) + shape)
+    for k, (a, b) in enumerate(idx):
+        P[a, b] = pi[k]; P[b, a] = pi[k]
+    Pn = np.einsum("ac...,bd...,cd...->ab...", L, L, P)
+    pin = np.stack([Pn[a, b] for (a, b) in idx])
+    return un, pin
+
+
+class ShiftedGubser:
+    """SURVEY 8c pin 5: the Gubser solution translated by (t0, z0) in the (t, z) plane.  Poincare invariance
+    makes it an exact solution of the same equations; seen from the unshifted Milne frame it has u~^eta != 0,
+    eta-gradients and every component of pi~ non-zero, so all Christoffel-born terms (Eq.24-26, 31, 35-38) act."""
+
+    def __init__(self, gubser, t0, z0):
+        self.g, self.t0, self.z0 = gubser, t0, z0
+
+    def fields(self, tau, X, Y, ETA):
+        t = tau * np.cosh(ETA) + self.t0
+        z = tau * np.sinh(ETA) + self.z0
+        taup = np.sqrt(t * t - z * z)
+        etap = np.arctanh(z / t)
+        e, u, pi = self.g.fields(taup, X, Y)
+        u, pi = boost_tilde(u, pi, etap - ETA)
+        return e, u, pi
