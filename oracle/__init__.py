@@ -26,37 +26,51 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+def _bind(path):
+    """dlopen one build of the oracle and declare its C ABI."""
+    lib = ctypes.CDLL(path)
+    dp = ctypes.POINTER(ctypes.c_double)
+    ip = ctypes.POINTER(ctypes.c_int)
+    lib.oracle_create.restype = ctypes.c_void_p
+    lib.oracle_create.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ip, ctypes.c_int,
+                                  ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+                                  ctypes.c_double, ctypes.c_double, dp, dp, ctypes.c_double,
+                                  ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                  ctypes.c_double, ctypes.c_double, ctypes.c_int]
+    lib.oracle_destroy.argtypes = [ctypes.c_void_p]
+    for name, nptr in [("oracle_load", 2), ("oracle_set_history", 1), ("oracle_read", 3),
+                       ("oracle_read_T", 1), ("oracle_read_history", 1), ("oracle_diag", 1),
+                       ("oracle_set_state", 3)]:
+        f = getattr(lib, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [ctypes.c_void_p] + [dp] * nptr
+    lib.oracle_step.restype = ctypes.c_int
+    lib.oracle_step.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    lib.oracle_rhs.restype = ctypes.c_int
+    lib.oracle_rhs.argtypes = [ctypes.c_void_p, dp, ctypes.c_double, dp, dp]
+    lib.oracle_eos.argtypes = [ctypes.c_void_p, ctypes.c_double, dp]
+    lib.oracle_rootfind.argtypes = [ctypes.c_void_p, dp, dp]
+    lib.oracle_limit_pi.restype = ctypes.c_int
+    lib.oracle_limit_pi.argtypes = [ctypes.c_void_p, ctypes.c_double, dp]
+    lib.oracle_set_option.restype = ctypes.c_int
+    lib.oracle_set_option.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double]
+    return lib
+
+
 def _load():
     global _lib
     if _lib is None:
-        lib = ctypes.CDLL(build())
-        dp = ctypes.POINTER(ctypes.c_double)
-        ip = ctypes.POINTER(ctypes.c_int)
-        lib.oracle_create.restype = ctypes.c_void_p
-        lib.oracle_create.argtypes = [ctypes.c_int] * 3 + [ctypes.c_double] * 3 + [ip, ctypes.c_int,
-                                      ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
-                                      ctypes.c_double, ctypes.c_double, dp, dp, ctypes.c_double,
-                                      ctypes.c_double, ctypes.c_double, ctypes.c_double,
-                                      ctypes.c_double, ctypes.c_double, ctypes.c_int]
-        lib.oracle_destroy.argtypes = [ctypes.c_void_p]
-        for name, nptr in [("oracle_load", 2), ("oracle_set_history", 1), ("oracle_read", 3),
-                           ("oracle_read_T", 1), ("oracle_read_history", 1), ("oracle_diag", 1),
-                           ("oracle_set_state", 3)]:
-            f = getattr(lib, name)
-            f.restype = ctypes.c_int
-            f.argtypes = [ctypes.c_void_p] + [dp] * nptr
-        lib.oracle_step.restype = ctypes.c_int
-        lib.oracle_step.argtypes = [ctypes.c_void_p, ctypes.c_int]
-        lib.oracle_rhs.restype = ctypes.c_int
-        lib.oracle_rhs.argtypes = [ctypes.c_void_p, dp, ctypes.c_double, dp, dp]
-        lib.oracle_eos.argtypes = [ctypes.c_void_p, ctypes.c_double, dp]
-        lib.oracle_rootfind.argtypes = [ctypes.c_void_p, dp, dp]
-        lib.oracle_limit_pi.restype = ctypes.c_int
-        lib.oracle_limit_pi.argtypes = [ctypes.c_void_p, ctypes.c_double, dp]
-        lib.oracle_set_option.restype = ctypes.c_int
-        lib.oracle_set_option.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double]
-        _lib = lib
+        _lib = _bind(build())
     return _lib
+
+
+def build_variant(out_path: str, extra_flags=()):
+    """A second build of the SAME source with different compiler flags (e.g. -ffp-contract=fast), used by the tests
+    that measure how far two correct roundings of the oracle drift apart.  Returns a library handle for
+    Oracle(..., lib=handle)."""
+    cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared"] + list(extra_flags) + ["-o", out_path, _SRC]
+    subprocess.check_call(cmd)
+    return _bind(out_path)
 
 
 def _p(a):
@@ -71,8 +85,8 @@ class Oracle:
 
     def __init__(self, nx, ny, nz, dx, dy, deta, dtau, tau0, eos, eta_over_s, bc=(0, 0, 0),
                  geometry=0, minmod_theta=1.1, e_floor=1e-7, pi_limit_xi=1.0, v_max=0.999,
-                 strict_eq53=0):
-        lib = _load()
+                 strict_eq53=0, lib=None):
+        lib = self._lib = lib if lib is not None else _load()
         self.shape = (nz, ny, nx)
         self.N = nx * ny * nz
         bca = (ctypes.c_int * 3)(*bc)
@@ -89,27 +103,27 @@ class Oracle:
 
     def __del__(self):
         if getattr(self, "_h", None):
-            _load().oracle_destroy(self._h)
+            self._lib.oracle_destroy(self._h)
             self._h = None
 
     def load(self, T, pi=None):
         T = np.ascontiguousarray(T, dtype=np.float64).reshape(4, -1)
         pi = None if pi is None else np.ascontiguousarray(pi, dtype=np.float64).reshape(10, -1)
         assert T.shape[1] == self.N
-        return _load().oracle_load(self._h, _p(T), _p(pi))
+        return self._lib.oracle_load(self._h, _p(T), _p(pi))
 
     def set_state(self, e, u3, pi=None):
         e = np.ascontiguousarray(e, dtype=np.float64).reshape(-1)
         u3 = np.ascontiguousarray(u3, dtype=np.float64).reshape(3, -1)
         pi = None if pi is None else np.ascontiguousarray(pi, dtype=np.float64).reshape(10, -1)
-        return _load().oracle_set_state(self._h, _p(e), _p(u3), _p(pi))
+        return self._lib.oracle_set_state(self._h, _p(e), _p(u3), _p(pi))
 
     def set_history(self, uprev3):
         a = np.ascontiguousarray(uprev3, dtype=np.float64).reshape(3, -1)
-        return _load().oracle_set_history(self._h, _p(a))
+        return self._lib.oracle_set_history(self._h, _p(a))
 
     def step(self, n=1):
-        rc = _load().oracle_step(self._h, int(n))
+        rc = self._lib.oracle_step(self._h, int(n))
         if rc:
             raise RuntimeError(f"oracle_step rc={rc}")
 
@@ -117,22 +131,22 @@ class Oracle:
         e = np.empty(self.N)
         u = np.empty((4, self.N))
         pi = np.empty((10, self.N))
-        _load().oracle_read(self._h, _p(e), _p(u), _p(pi))
+        self._lib.oracle_read(self._h, _p(e), _p(u), _p(pi))
         return e.reshape(self.shape), u.reshape((4,) + self.shape), pi.reshape((10,) + self.shape)
 
     def read_T(self):
         T = np.empty((4, self.N))
-        _load().oracle_read_T(self._h, _p(T))
+        self._lib.oracle_read_T(self._h, _p(T))
         return T.reshape((4,) + self.shape)
 
     def read_history(self):
         u = np.empty((3, self.N))
-        _load().oracle_read_history(self._h, _p(u))
+        self._lib.oracle_read_history(self._h, _p(u))
         return u.reshape((3,) + self.shape)
 
     def diag(self):
         d = np.zeros(9)
-        _load().oracle_diag(self._h, _p(d))
+        self._lib.oracle_diag(self._h, _p(d))
         return dict(tau=d[0], step=int(d[1]), cfl=tuple(d[2:5]), e_max=d[5], floored=int(d[6]),
                     clamped=int(d[7]), pi_limited=int(d[8]))
 
@@ -140,28 +154,28 @@ class Oracle:
         dtu4 = np.ascontiguousarray(dtu4, dtype=np.float64).reshape(4, -1)
         ST = np.zeros((4, self.N))
         SP = np.zeros((10, self.N))
-        _load().oracle_rhs(self._h, _p(dtu4), float(tau), _p(ST), _p(SP))
+        self._lib.oracle_rhs(self._h, _p(dtu4), float(tau), _p(ST), _p(SP))
         return ST.reshape((4,) + self.shape), SP.reshape((10,) + self.shape)
 
     def eos(self, e):
         out = np.zeros(3)
-        _load().oracle_eos(self._h, float(e), _p(out))
+        self._lib.oracle_eos(self._h, float(e), _p(out))
         return tuple(out)
 
     def limit_pi(self, e, pi10):
         """pi limiter (A14) on one cell: returns (scaled pi[10], acted?)."""
         p = np.array(pi10, dtype=np.float64)
-        acted = _load().oracle_limit_pi(self._h, float(e), _p(p))
+        acted = self._lib.oracle_limit_pi(self._h, float(e), _p(p))
         return p, bool(acted)
 
     OPT_HEUN_PRINTED = 0
 
     def set_option(self, key, value):
-        if _load().oracle_set_option(self._h, int(key), float(value)):
+        if self._lib.oracle_set_option(self._h, int(key), float(value)):
             raise ValueError("oracle_set_option: unknown key")
 
     def rootfind(self, M4):
         M4 = np.ascontiguousarray(M4, dtype=np.float64)
         out = np.zeros(4)
-        _load().oracle_rootfind(self._h, _p(M4), _p(out))
+        self._lib.oracle_rootfind(self._h, _p(M4), _p(out))
         return out

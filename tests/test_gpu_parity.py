@@ -94,14 +94,23 @@ def test_small_event_fp64(crossover, kernel, eta_s, moving):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_small_event_fp32(crossover, kernel):
+    """fp32 bar (L2 <= 2e-4) after 10 steps.  Why 10 and not 20: the dilute rim of this 40x36x24 box is clamped to the
+    v_max limit from step ~3 on (5 800 clamp events in 12 steps), and from there on any two roundings of the algorithm
+    diverge -- the oracle against its own FMA-contracted build does the same (tests/test_gpu_longrun.py,
+    test_moving_event_drift_is_rounding_chaos).  Measured at 20 steps (round 2, B200): L2(e) 1.4e-3 .. 4.1e-3, asserted
+    below as bounded; on the event that never clamps the fp32 path stays at 9e-7 for 100 steps
+    (test_static_event_100_steps)."""
     cfg = small_parton_config(eta_over_s=0.08, moving=True, steps=10)
     T, _ = inputs.ic_partons(cfg, inputs.seed_for(3))
     o, g = run_pair(cfg, crossover, T, None, 0, gkw=dict(kernel=kernel, precision=32))
     o.step(cfg.steps); g.step(cfg.steps)
     er = errors(crossover, o.read(), g.read())
-    print("small event fp32", er)
+    print("small event fp32, 10 steps", er)
     assert er["l2_e"] <= 2e-4 and er["l2_T"] <= 2e-4
-    assert g.diag()["nan"] == 0
+    o.step(10); g.step(10)
+    er = errors(crossover, o.read(), g.read())
+    print("small event fp32, 20 steps", er)
+    assert er["l2_e"] <= 2e-2 and g.diag()["nan"] == 0
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
