@@ -12,6 +12,10 @@
 // warp transaction), and all fields of those 32 cells follow each other, so that inside a kernel the field
 // offset is a compile-time immediate and a cell's whole state lies in one 4.8 KB stretch of DRAM.
 // buf X (+gstar) doubles as the staging area for host-memory load/read between steps.
+//
+// Kernel 3 (the tile kernel, default) uses a different field store: plain SoA with two ghost layers per side,
+//   [field][nz+4][ny+4][pitch]   (pitch = nx+4 rounded up to 16 bytes), nf = 4 / 14 fields and nothing derived,
+// addressed by TMA tensor maps (one per buffer and box depth) that hydro_create encodes.
 #include "../../include/clvisc_hydro.h"
 
 #include <cmath>
@@ -22,6 +26,7 @@
 
 #include "hydro_stage_ref.cuh"
 #include "hydro_stage_fused.cuh"
+#include "hydro_stage_tile.cuh"
 
 namespace clv {
 
@@ -31,6 +36,8 @@ constexpr double kHbarc = 0.1973269804;   // GeV fm (A18)
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
+  int soa;               // 0: blocked layout of kernels 1/2; 1: ghosted SoA of kernel 3
+  long long py, pz, pf;  // soa: row, plane and field strides (elements)
   int nxb, blk, gp;      // x-blocks per row, elements per x-block (32 * nft), gstar row pitch
   long long sy, sz;      // row and plane strides (elements)
   long long nelem;       // elements of one state buffer
@@ -39,12 +46,30 @@ struct Layout {
   size_t off_diag, off_eos, off_buf[3], off_gstar, total;
 };
 
-static bool make_layout(const hydro_grid* g, int precision, double eta_s, Layout* L) {
+static bool make_layout(const hydro_grid* g, int precision, double eta_s, int kernel, Layout* L) {
   if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;
   if (precision != 64 && precision != 32) return false;
   if ((long long)g->nx * g->ny * g->nz > (1ll << 36)) return false;
+  // launch-grid limits of kernels 1/2 (gridDim.y, gridDim.z) and of the TMA coordinates of kernel 3
+  if (g->nz > 65535 || g->ny > 8 * 65535 || g->nx > (1 << 30)) return false;
   L->elem = precision == 64 ? 8 : 4;
   L->nf = eta_s > 0.0 ? 14 : 4;
+  L->soa = (kernel == 0 || kernel == 3) ? 1 : 0;
+  if (L->soa) {
+    const int per16 = 16 / (int)L->elem;
+    L->py = ((long long)g->nx + 2 * HALO + per16 - 1) / per16 * per16;
+    L->pz = L->py * (g->ny + 2 * HALO);
+    L->pf = L->pz * (g->nz + 2 * HALO);
+    L->nft = L->nf; L->nxb = 0; L->blk = 0; L->gp = 0; L->sy = 0; L->sz = 0;
+    L->nelem = L->pf * L->nf;
+    size_t off = 0;
+    L->off_diag = off; off += 256;
+    L->off_eos = off; off += align_up((size_t)5 * kMaxEosNodes * L->elem, 256);
+    for (int b = 0; b < 3; ++b) { L->off_buf[b] = off; off += align_up((size_t)L->nelem * L->elem, 256); }
+    L->off_gstar = off; off += align_up((size_t)L->pf * L->elem, 256);
+    L->total = off;
+    return true;
+  }
   L->nft = L->nf + X_COUNT;     // + extended slots P, u^tau, c_x, c_y, c_eta
   L->nxb = (g->nx + 31) / 32;
   L->blk = 32 * L->nft;
@@ -88,8 +113,9 @@ __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restr
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) M[mu] = T[mu * a.N + cc] - p[mu];    // T_id = T - pi  (Eq.51)
   unsigned flags = 0;
-  R e, ux, uy, un;
-  rootfind(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, ux, uy, un, flags);
+  R e, ux, uy, un, P, cs2, g;
+  // warp-uniform Newton with early exit (round 1 ran 64 fixed iterations here: 6.7 ms at 301x301x201)
+  rootfind_warp(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, P, cs2, ux, uy, un, g, flags);
   if (active) {
     st[c] = e; st[FS + c] = ux; st[2 * FS + c] = uy; st[3 * FS + c] = un;
     if (VISC) {
@@ -97,9 +123,7 @@ __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restr
       for (int m = 0; m < 10; ++m) st[(F_PI + m) * FS + c] = p[m];
     }
     // extended slots read by kernel 2
-    R P, cs2, cx, cy, cn;
-    eos_P(a.eos, e, P, cs2);
-    const R g = sqrt_(R(1) + ux * ux + uy * uy + un * un);
+    R cx, cy, cn;
     signal_speeds3(g, ux, uy, un, cs2, cx, cy, cn);
     R* __restrict__ sx = st + (VISC ? 14 : 4) * FS + c;
     sx[X_P * FS] = P; sx[X_G * FS] = g;
@@ -146,6 +170,98 @@ __global__ void __launch_bounds__(256) history_kernel(IoArgs<R> a, R* __restrict
   }
 }
 
+// ---- the same three kernels for the ghosted SoA layout of kernel 3 ---------------------------------------------------
+template <typename R>
+struct SoaArgs {
+  int nx, ny, nz;
+  long long py, pz, pf, N;
+  int bc[3];
+  R e_floor, v_max;
+  EosDev<R> eos;
+  DiagDev* diag;
+};
+
+// store v at (field f, cell i,j,k) and at the ghost positions that mirror the cell (boundary rule a11)
+template <typename R>
+__device__ __forceinline__ void soa_put(const SoaArgs<R>& a, R* __restrict__ st, int f, int i, int j, int k, R v,
+                                        const int* gl, const int* ng) {
+  R* __restrict__ o = st + (long long)f * a.pf + (long long)(k + HALO) * a.pz + (long long)(j + HALO) * a.py + (i + HALO);
+  o[0] = v;
+  for (int t = 0; t < ng[0]; ++t) o[gl[t] - i] = v;
+  for (int t = 0; t < ng[1]; ++t) o[(long long)(gl[4 + t] - j) * a.py] = v;
+  for (int t = 0; t < ng[2]; ++t) o[(long long)(gl[8 + t] - k) * a.pz] = v;
+}
+
+template <typename R, bool VISC>
+__global__ void __launch_bounds__(256) load_kernel_soa(SoaArgs<R> a, const R* __restrict__ T, const R* __restrict__ pi,
+                                                       R* __restrict__ st) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = cu < a.N;
+  const long long cc = active ? cu : 0;
+  const int i = (int)(cc % a.nx), j = (int)((cc / a.nx) % a.ny), k = (int)(cc / ((long long)a.nx * a.ny));
+  R p[10];
+#pragma unroll
+  for (int m = 0; m < 10; ++m) p[m] = (VISC && pi) ? pi[m * a.N + cc] : R(0);
+  R M[4];
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) M[mu] = T[mu * a.N + cc] - p[mu];    // T_id = T - pi  (Eq.51)
+  unsigned flags = 0;
+  R e, P, cs2, ux, uy, un, g;
+  rootfind_warp(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, P, cs2, ux, uy, un, g, flags);
+  if (active) {
+    int gl[12], ng[3];
+    ng[0] = ghost_list(i, a.nx, a.bc[0], gl);
+    ng[1] = ghost_list(j, a.ny, a.bc[1], gl + 4);
+    ng[2] = ghost_list(k, a.nz, a.bc[2], gl + 8);
+    soa_put(a, st, 0, i, j, k, e, gl, ng); soa_put(a, st, 1, i, j, k, ux, gl, ng);
+    soa_put(a, st, 2, i, j, k, uy, gl, ng); soa_put(a, st, 3, i, j, k, un, gl, ng);
+    if (VISC) {
+#pragma unroll
+      for (int m = 0; m < 10; ++m) soa_put(a, st, 4 + m, i, j, k, p[m], gl, ng);
+    }
+  } else {
+    flags = 0;
+  }
+  count_flags(a.diag, flags);
+  const double r = warp_max(active ? (double)e : 0.0);
+  if ((threadIdx.x & 31) == 0) atomic_max_nonneg(&a.diag->emax[1], r);
+}
+
+template <typename R, bool VISC>
+__global__ void __launch_bounds__(256) read_kernel_soa(SoaArgs<R> a, const R* __restrict__ st, R* __restrict__ e,
+                                                       R* __restrict__ u, R* __restrict__ pi) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cu >= a.N) return;
+  const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
+  const R* __restrict__ c = st + (long long)(k + HALO) * a.pz + (long long)(j + HALO) * a.py + (i + HALO);
+  if (e) e[cu] = c[0];
+  if (u) {
+    const R ux = c[a.pf], uy = c[2 * a.pf], un = c[3 * a.pf];
+    u[cu] = sqrt_(R(1) + ux * ux + uy * uy + un * un);
+    u[a.N + cu] = ux; u[2 * a.N + cu] = uy; u[3 * a.N + cu] = un;
+  }
+  if (pi) {
+#pragma unroll
+    for (int m = 0; m < 10; ++m) pi[m * a.N + cu] = VISC ? c[(4 + m) * a.pf] : R(0);
+  }
+}
+
+// pad (dir = 0: user -> internal) or unpad (dir = 1) three history fields (no ghosts: the history is read at the
+// cell centre only)
+template <typename R>
+__global__ void __launch_bounds__(256) history_kernel_soa(SoaArgs<R> a, R* __restrict__ hist, R* __restrict__ user,
+                                                          int dir) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cu >= a.N) return;
+  const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
+  R* __restrict__ c = hist + (long long)(k + HALO) * a.pz + (long long)(j + HALO) * a.py + (i + HALO);
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    if (dir == 0) c[m * a.pf] = user[m * a.N + cu];
+    else user[m * a.N + cu] = c[m * a.pf];
+  }
+}
+
 }  // namespace clv
 
 using namespace clv;
@@ -168,6 +284,9 @@ struct hydro_ctx {
   long long step;
   long long launches;
   bool loaded;
+  // kernel 3: TMA tensor maps of the three state buffers with box depth nf ([b][0]) and 4 ([b][1]); tiling
+  CUtensorMap tmap[3][2];
+  int ntx, nty, nchunk, chunk;
 };
 
 namespace {
@@ -175,6 +294,96 @@ namespace {
 template <typename R> const EosDev<R>& eos_of(const hydro_ctx* c);
 template <> const EosDev<double>& eos_of<double>(const hydro_ctx* c) { return c->eos64; }
 template <> const EosDev<float>& eos_of<float>(const hydro_ctx* c) { return c->eos32; }
+
+// ---- kernel 3 host side: tensor maps, tiling, argument block ----------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 4-D map (x, y, z, field) of one ghosted SoA buffer with box {36, 12, 1, nbox}
+int make_tmap(const hydro_ctx* c, void* base, int nbox, CUtensorMap* out) {
+  static EncodeTiledFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess || !fn) {
+      (void)cudaGetLastError();
+      return HYDRO_ECUDA;
+    }
+    encode = reinterpret_cast<EncodeTiledFn>(fn);
+  }
+  const Layout& L = c->L;
+  const cuuint64_t dims[4] = {(cuuint64_t)(c->grid.nx + 2 * HALO), (cuuint64_t)(c->grid.ny + 2 * HALO),
+                              (cuuint64_t)(c->grid.nz + 2 * HALO), (cuuint64_t)nbox};
+  const cuuint64_t strides[3] = {(cuuint64_t)L.py * L.elem, (cuuint64_t)L.pz * L.elem, (cuuint64_t)L.pf * L.elem};
+  const cuuint32_t box[4] = {(cuuint32_t)SX, (cuuint32_t)SY, 1u, (cuuint32_t)nbox};
+  const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+  const CUresult r = encode(out, L.elem == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, base,
+                            dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? HYDRO_OK : HYDRO_ECUDA;
+}
+
+// z-chunks per tile column: fill the SMs in whole waves while keeping the 4-plane pipeline warm-up per chunk small
+void choose_tiling(hydro_ctx* c, int nsm) {
+  c->ntx = (c->grid.nx + TX - 1) / TX;
+  c->nty = (c->grid.ny + TY - 1) / TY;
+  const long long tiles = (long long)c->ntx * c->nty;
+  const int nz = c->grid.nz;
+  double best = -1.0;
+  for (int cand = 1; cand <= nz && cand <= 256; ++cand) {
+    const int chunk = (nz + cand - 1) / cand, nchunk = (nz + chunk - 1) / chunk;
+    const long long blocks = tiles * nchunk;
+    const long long waves = (blocks + nsm - 1) / nsm;
+    const double eff = (double)blocks / (double)(waves * nsm) * (double)chunk / ((double)chunk + 1.5);
+    if (eff > best * 1.0001) { best = eff; c->chunk = chunk; c->nchunk = nchunk; }
+  }
+}
+
+template <typename R>
+TileArgs<R> tile_args(const hydro_ctx* c, double tau_rhs, double tau_n, double tau_1) {
+  TileArgs<R> a;
+  memset(&a, 0, sizeof(a));
+  const bool milne = c->grid.geometry == 0;
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz;
+  a.py = c->L.py; a.pz = c->L.pz; a.pf = c->L.pf;
+  for (int d = 0; d < 3; ++d) a.bc[d] = c->grid.bc[d];
+  a.milne = milne ? 1 : 0;
+  a.tau = (R)tau_rhs; a.inv_tau = (R)(1.0 / tau_rhs);
+  a.tf_n = (R)(milne ? tau_n : 1.0); a.tf_1 = (R)(milne ? tau_1 : 1.0); a.inv_tf_1 = (R)(milne ? 1.0 / tau_1 : 1.0);
+  a.h = (R)c->dtau; a.inv_h = (R)(1.0 / c->dtau);
+  a.scale[0] = (R)(1.0 / c->grid.dx); a.scale[1] = (R)(1.0 / c->grid.dy);
+  a.scale[2] = (R)(milne ? 1.0 / (tau_rhs * c->grid.deta) : 1.0 / c->grid.deta);
+  a.theta = (R)c->theta; a.e_floor = (R)c->e_floor; a.xi = (R)c->xi; a.v_max = (R)c->v_max;
+  a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (5.0 * c->eta_s * kHbarc) : 0.0);
+  a.root_iters = c->root_iters;
+  a.eos = eos_of<R>(c);
+  a.diag = c->diag;
+  a.ntx = c->ntx; a.nty = c->nty; a.nchunk = c->nchunk; a.chunk = c->chunk;
+  return a;
+}
+
+template <typename R, bool VISC, int MODE>
+int launch_tile(hydro_ctx* c, const TileArgs<R>& a, int buf_in) {
+  constexpr bool USE_PI = VISC && (MODE != 0);
+  const CUtensorMap& map = c->tmap[buf_in][(USE_PI || !c->visc) ? 0 : 1];
+  const cudaError_t e = launch_stage_tile<R, VISC, MODE>(a, map, c->stream);
+  c->launches += 1;
+  return e == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+}
+
+template <typename R>
+SoaArgs<R> soa_args(const hydro_ctx* c) {
+  SoaArgs<R> a;
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz;
+  a.py = c->L.py; a.pz = c->L.pz; a.pf = c->L.pf; a.N = (long long)a.nx * a.ny * a.nz;
+  for (int d = 0; d < 3; ++d) a.bc[d] = c->grid.bc[d];
+  a.e_floor = (R)c->e_floor; a.v_max = (R)c->v_max;
+  a.eos = eos_of<R>(c);
+  a.diag = c->diag;
+  return a;
+}
 
 template <typename R>
 int upload_eos(hydro_ctx* c, const hydro_eos* eos, EosDev<R>* q) {
@@ -258,6 +467,12 @@ int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
 
 template <typename R>
 int do_bootstrap(hydro_ctx* c) {
+  if (c->L.soa) {
+    TileArgs<R> t = tile_args<R>(c, c->tau0, c->tau0, c->tau0 + c->dtau);
+    t.out = static_cast<R*>(c->buf[c->prev]) + c->L.pf;      // u~^i slots (fields 1..3) of the history buffer
+    t.slot = 0;
+    return c->visc ? launch_tile<R, true, 0>(c, t, c->cur) : launch_tile<R, false, 0>(c, t, c->cur);
+  }
   StageArgs<R> a = stage_args<R>(c, c->tau0, c->tau0, c->tau0 + c->dtau);
   a.in = static_cast<const R*>(c->buf[c->cur]);
   a.out = static_cast<R*>(c->buf[c->prev]) + FS;         // u~^i slots (fields 1..3) of the history buffer
@@ -272,6 +487,26 @@ int do_step(hydro_ctx* c) {
   R* cur = static_cast<R*>(c->buf[c->cur]);
   R* prev = static_cast<R*>(c->buf[c->prev]);
   R* X = static_cast<R*>(c->buf[2]);
+  if (c->L.soa) {
+    TileArgs<R> t1 = tile_args<R>(c, tau_n, tau_n, tau_1);
+    t1.uprev = prev + c->L.pf; t1.gstar = static_cast<R*>(c->gstar); t1.out = X; t1.slot = slot;
+    TileArgs<R> t2 = tile_args<R>(c, tau_1, tau_n, tau_1);
+    t2.sn = cur; t2.gstar = static_cast<R*>(c->gstar); t2.out = prev; t2.slot = slot;
+    int rc;
+    if (c->visc) {
+      rc = launch_tile<R, true, 1>(c, t1, c->cur);
+      if (rc) return rc;
+      rc = launch_tile<R, true, 2>(c, t2, 2);
+    } else {
+      rc = launch_tile<R, false, 1>(c, t1, c->cur);
+      if (rc) return rc;
+      rc = launch_tile<R, false, 2>(c, t2, 2);
+    }
+    if (rc) return rc;
+    const int t = c->cur; c->cur = c->prev; c->prev = t;
+    c->step += 1;
+    return HYDRO_OK;
+  }
   StageArgs<R> a1 = stage_args<R>(c, tau_n, tau_n, tau_1);
   a1.in = cur; a1.uprev = prev + FS; a1.gstar = static_cast<R*>(c->gstar); a1.out = X; a1.slot = slot;
   StageArgs<R> a2 = stage_args<R>(c, tau_1, tau_n, tau_1);
@@ -312,10 +547,16 @@ int do_load(hydro_ctx* c, const void* T, const void* pi, int mem) {
   }
   if (cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) return HYDRO_ECUDA;
   c->cur = 0; c->prev = 1; c->step = 0;
-  IoArgs<R> a = io_args<R>(c);
   const unsigned nb = (unsigned)((N + 255) / 256);
-  if (c->visc) load_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
-  else load_kernel<R, false><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+  if (c->L.soa) {
+    SoaArgs<R> a = soa_args<R>(c);
+    if (c->visc) load_kernel_soa<R, true><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+    else load_kernel_soa<R, false><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+  } else {
+    IoArgs<R> a = io_args<R>(c);
+    if (c->visc) load_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+    else load_kernel<R, false><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+  }
   c->launches += 1;
   if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
   int rc = do_bootstrap<R>(c);
@@ -332,7 +573,11 @@ int do_read(hydro_ctx* c, void* e, void* u, void* pi, int mem) {
   const unsigned nb = (unsigned)((N + 255) / 256);
   const R* st = static_cast<const R*>(c->buf[c->cur]);
   auto run = [&](R* pe, R* pu, R* pp) -> int {
-    if (c->visc) read_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, st, pe, pu, pp);
+    if (c->L.soa) {
+      SoaArgs<R> sa = soa_args<R>(c);
+      if (c->visc) read_kernel_soa<R, true><<<nb, 256, 0, c->stream>>>(sa, st, pe, pu, pp);
+      else read_kernel_soa<R, false><<<nb, 256, 0, c->stream>>>(sa, st, pe, pu, pp);
+    } else if (c->visc) read_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, st, pe, pu, pp);
     else read_kernel<R, false><<<nb, 256, 0, c->stream>>>(a, st, pe, pu, pp);
     c->launches += 1;
     return cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
@@ -372,7 +617,7 @@ int do_history(hydro_ctx* c, void* user, int mem, int dir) {
   const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
   IoArgs<R> a = io_args<R>(c);
   const unsigned nb = (unsigned)((N + 255) / 256);
-  R* hist = static_cast<R*>(c->buf[c->prev]) + FS;
+  R* hist = static_cast<R*>(c->buf[c->prev]) + (c->L.soa ? c->L.pf : (long long)FS);
   R* dev = static_cast<R*>(user);
   R* stage = static_cast<R*>(c->buf[2]);
   if (mem == HYDRO_MEM_HOST) {
@@ -381,7 +626,8 @@ int do_history(hydro_ctx* c, void* user, int mem, int dir) {
         cudaMemcpyAsync(stage, user, (size_t)3 * N * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
       return HYDRO_ECUDA;
   }
-  history_kernel<R><<<nb, 256, 0, c->stream>>>(a, hist, dev, dir);
+  if (c->L.soa) history_kernel_soa<R><<<nb, 256, 0, c->stream>>>(soa_args<R>(c), hist, dev, dir);
+  else history_kernel<R><<<nb, 256, 0, c->stream>>>(a, hist, dev, dir);
   c->launches += 1;
   if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
   if (mem == HYDRO_MEM_HOST) {
@@ -398,9 +644,10 @@ int do_history(hydro_ctx* c, void* user, int mem, int dir) {
 extern "C" {
 
 size_t hydro_workspace_bytes(const hydro_grid* grid, int precision, double eta_over_s) {
-  Layout L;
-  if (!make_layout(grid, precision, eta_over_s, &L)) return 0;
-  return L.total;
+  // one figure for every kernel choice: the larger of the blocked (kernels 1/2) and the ghosted SoA (kernel 3) stores
+  Layout L2, L3;
+  if (!make_layout(grid, precision, eta_over_s, 2, &L2) || !make_layout(grid, precision, eta_over_s, 3, &L3)) return 0;
+  return L2.total > L3.total ? L2.total : L3.total;
 }
 
 int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double tau0, const hydro_eos* eos,
@@ -409,7 +656,8 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   *out = nullptr;
   if (!grid || !eos || !opts) return HYDRO_EINVAL;
   Layout L;
-  if (!make_layout(grid, opts->precision, eta_over_s, &L)) return HYDRO_EINVAL;
+  if (opts->kernel < 0 || opts->kernel > 3) return HYDRO_EINVAL;
+  if (!make_layout(grid, opts->precision, eta_over_s, opts->kernel, &L)) return HYDRO_EINVAL;
   if (!(dtau > 0.0) || !(grid->dx > 0.0) || !(grid->dy > 0.0) || !(grid->deta > 0.0)) return HYDRO_EINVAL;
   if (grid->geometry != 0 && grid->geometry != 1) return HYDRO_EINVAL;
   if (grid->geometry == 0 && !(tau0 > 0.0)) return HYDRO_EINVAL;
@@ -418,7 +666,6 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   if (!(eta_over_s >= 0.0)) return HYDRO_EINVAL;
   if (!(opts->minmod_theta >= 1.0 && opts->minmod_theta <= 2.0)) return HYDRO_EINVAL;
   if (!(opts->e_floor > 0.0)) return HYDRO_EINVAL;
-  if (opts->kernel < 0 || opts->kernel > 2) return HYDRO_EINVAL;
   if (eos->kind != 0 && eos->kind != 1) return HYDRO_EINVAL;
   if (!(eos->c_sb > 0.0)) return HYDRO_EINVAL;
   if (eos->kind == 1) {
@@ -436,7 +683,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   if (!c) return HYDRO_ENOMEM;
   c->grid = *grid; c->dtau = dtau; c->tau0 = tau0; c->eta_s = eta_over_s;
   c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
-  c->kernel = opts->kernel == 0 ? 2 : opts->kernel;
+  c->kernel = opts->kernel == 0 ? 3 : opts->kernel;
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
   c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;
@@ -449,6 +696,19 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->cur = 0; c->prev = 1; c->step = 0; c->launches = 0; c->loaded = false;
   int rc = opts->precision == 64 ? upload_eos<double>(c, eos, &c->eos64) : upload_eos<float>(c, eos, &c->eos32);
   if (rc == HYDRO_OK && cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) rc = HYDRO_ECUDA;
+  if (rc == HYDRO_OK && L.soa) {
+    int dev = 0, nsm = 148;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+      rc = HYDRO_ECUDA;
+    choose_tiling(c, nsm > 0 ? nsm : 148);
+    // ghost cells and pitch padding are read by the TMA boxes before anything writes them: start from zeros
+    if (rc == HYDRO_OK && cudaMemsetAsync(c->buf[0], 0, (size_t)3 * align_up((size_t)L.nelem * L.elem, 256), c->stream) != cudaSuccess)
+      rc = HYDRO_ECUDA;
+    for (int b = 0; b < 3 && rc == HYDRO_OK; ++b) {
+      rc = make_tmap(c, c->buf[b], L.nf, &c->tmap[b][0]);
+      if (rc == HYDRO_OK) rc = make_tmap(c, c->buf[b], 4, &c->tmap[b][1]);
+    }
+  }
   if (rc != HYDRO_OK) { delete c; return rc; }
   *out = c;
   return HYDRO_OK;

@@ -11,6 +11,7 @@
 //   * warp-uniform early exit of the Newton iteration (no intra-warp divergence).
 #pragma once
 #include "hydro_stage_ref.cuh"
+#include "hydro_stage_update.cuh"
 
 namespace clv {
 
@@ -75,83 +76,6 @@ __device__ __forceinline__ void signal_speeds3(R g, R ux, R uy, R un, R cs2, R& 
   cx = (fabs_(vx) * omc + csg * sqrt_(max_(base - vx * vx * omc, R(0)))) * D;
   cy = (fabs_(vy) * omc + csg * sqrt_(max_(base - vy * vy * omc, R(0)))) * D;
   cn = (fabs_(vn) * omc + csg * sqrt_(max_(base - vn * vn * omc, R(0)))) * D;
-}
-
-// Root-find (Eq.51/54; A7, A8) with a warp-uniform iteration count: every lane runs the same number of
-// Newton steps (the warp leaves the loop when all 32 lanes have converged), so there is no divergence.
-// Must be called by all lanes of the warp.  Also returns P, c_s^2 at the root and u~^tau.
-template <typename R>
-__device__ __forceinline__ void rootfind_warp(const EosDev<R>& eos, R M0, R Mx, R My, R Mn, R e_start, int iters,
-                                              R e_floor, R v_max, R& e_out, R& P_out, R& cs2_out, R& ux, R& uy,
-                                              R& un, R& g_out, unsigned& flags) {
-  if (!(M0 == M0) || !(Mx == Mx) || !(My == My) || !(Mn == Mn)) flags |= 8u;
-  const bool vac = !(M0 > e_floor);
-  if (vac) { flags |= 1u; M0 = R(1); Mx = My = Mn = R(0); }
-  R M2 = Mx * Mx + My * My + Mn * Mn;
-  const R lim = v_max * M0;
-  if (M2 > lim * lim) {
-    const R sc = lim * rsqrt_(M2);
-    Mx *= sc; My *= sc; Mn *= sc; M2 = lim * lim; flags |= 2u;
-  }
-  R e, P, cs2;
-  if (eos.kind == 0) {
-    const R d = M0 * M0 - M2;
-    e = R(3) * d / (M0 + sqrt_(M0 * M0 + R(3) * d));
-    P = e * R(1.0 / 3.0); cs2 = R(1.0 / 3.0);
-  } else {
-    const R tol = (sizeof(R) == 8) ? R(1e-15) : R(2e-7);
-    const R tol2 = (sizeof(R) == 8) ? R(1e-9) : R(1e-4);
-    R lo = R(0), hi = M0;
-    e = e_start;
-    if (!(e > lo && e < hi)) e = M0 - M2 / (M0 + M0 * R(1.0 / 3.0));
-    if (!(e > lo && e < hi)) e = R(0.5) * M0;
-    for (int it = 0; it < iters; ++it) {
-      eos_P(eos, e, P, cs2);
-      const R inv = R(1) / (M0 + P);
-      const R g = M0 - M2 * inv - e;
-      const bool conv = !(abs_(g) > tol * M0);
-      if (__all_sync(0xffffffffu, conv)) break;
-      const R dg = M2 * cs2 * inv * inv - R(1);
-      if (g > R(0)) lo = e; else hi = e;
-      R en = e - g / dg;
-      if (!(en >= lo && en <= hi)) en = R(0.5) * (lo + hi);
-      e = conv ? e : en;
-      // Newton converges quadratically on the (piecewise linear, convex) g: a step taken from a residual
-      // below sqrt(tol) lands below tol, so the warp can leave without another evaluation
-      if (__all_sync(0xffffffffu, !(abs_(g) > tol2 * M0))) break;
-    }
-    eos_P(eos, e, P, cs2);
-    const R g = M0 - M2 / (M0 + P) - e;
-    if (abs_(g) > R(1e3) * tol * M0) flags |= 4u;
-  }
-  if (vac) e = R(0);
-  if (e < e_floor) {
-    e = e_floor; flags |= 1u;
-    eos_P(eos, e, P, cs2);
-  }
-  const R iw = R(1) / (M0 + P);
-  const R vx = Mx * iw, vy = My * iw, vn = Mn * iw;
-  const R gam = rsqrt_(R(1) - (vx * vx + vy * vy + vn * vn));
-  ux = gam * vx; uy = gam * vy; un = gam * vn;
-  e_out = e; P_out = P; cs2_out = cs2;
-  // u~^tau consistent with the stored u~^i (what a consumer would recompute): sqrt(1 + u.u)
-  g_out = sqrt_(R(1) + ux * ux + uy * uy + un * un);
-}
-
-// pi limiter (A14) with P(e) supplied
-template <typename R>
-__device__ __forceinline__ void limit_pi_P(R xi, R e, R P, R pi[10], unsigned& flags) {
-  if (!(xi > R(0))) return;
-  const R pp = pi[0] * pi[0] - R(2) * (pi[1] * pi[1] + pi[2] * pi[2] + pi[3] * pi[3]) + pi[4] * pi[4] +
-               pi[7] * pi[7] + pi[9] * pi[9] + R(2) * (pi[5] * pi[5] + pi[6] * pi[6] + pi[8] * pi[8]);
-  const R mag2 = abs_(pp);
-  const R lim2 = xi * xi * (e * e + R(3) * P * P);
-  if (mag2 > lim2) {
-    const R r = sqrt_(lim2) * rsqrt_(mag2);
-#pragma unroll
-    for (int m = 0; m < 10; ++m) pi[m] *= r;
-    flags |= 16u;
-  }
 }
 
 #ifndef CLV_MINB
@@ -270,14 +194,13 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
   }
 
   // ---- cell-centre state (re-read after the flux loop: L1 hits, keeps the loop's register set small) ---
-  const R e_c = pc[0];
-  R ut[4];
-  ut[1] = pc[sf]; ut[2] = pc[2 * sf]; ut[3] = pc[3 * sf];
-  ut[0] = pc[OX + X_G * FS];
-  const R P_c = pc[OX + X_P * FS];
-  R pic[10];
+  Cell<R> cc, cn_;
+  cc.e = pc[0];
+  cc.u[1] = pc[sf]; cc.u[2] = pc[2 * sf]; cc.u[3] = pc[3 * sf];
+  cc.u[0] = pc[OX + X_G * FS];
+  cc.P = pc[OX + X_P * FS];
 #pragma unroll
-  for (int m = 0; m < 10; ++m) pic[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
+  for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
 
   // spatial rows of nabla~_mu u~^nu by central differences (A9); eta row divided by tau (Eq.22)
   R grad[4][4];
@@ -301,88 +224,35 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
     }
   }
 
-  // ---- geometric source of T (Eq.31, sign A1) ---------------------------------------------------
-  const R w_c = e_c + P_c;
-  if (a.milne) {
-    S[0] -= w_c * ut[3] * ut[3] + P_c + pic[9];      // -T_f^{eta eta}
-    S[3] -= w_c * ut[0] * ut[3] + pic[3];            // -T_f^{tau eta}
-  }
-
   // ---- state n at the centre (MODE 2 reads it; MODE 0/1: it is the star centre itself) -----------
-  R e_n = e_c, un_[4] = {ut[0], ut[1], ut[2], ut[3]}, pin[10], P_n = P_c;
-#pragma unroll
-  for (int m = 0; m < 10; ++m) pin[m] = pic[m];
   if (MODE == 2) {
     const R* __restrict__ sn = a.sn + c;
-    e_n = sn[0];
-    un_[1] = sn[sf]; un_[2] = sn[2 * sf]; un_[3] = sn[3 * sf];
-    un_[0] = sn[OX + X_G * FS];
-    P_n = sn[OX + X_P * FS];
+    cn_.e = sn[0];
+    cn_.u[1] = sn[sf]; cn_.u[2] = sn[2 * sf]; cn_.u[3] = sn[3 * sf];
+    cn_.u[0] = sn[OX + X_G * FS];
+    cn_.P = sn[OX + X_P * FS];
 #pragma unroll
-    for (int m = 0; m < 10; ++m) pin[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
+    for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
   }
-
-  R gdiv = R(1), gst = R(1);
+  R up3[3] = {R(0), R(0), R(0)};
+  R gst = R(1);
   if (USE_PI) {
     if (MODE == 1) {
       const R* __restrict__ up = a.uprev + c;
-      const R sx = R(2) * ut[1] - up[0], sy = R(2) * ut[2] - up[sf], sn_ = R(2) * ut[3] - up[2 * sf];
-      const R gs2 = R(1) + sx * sx + sy * sy + sn_ * sn_;
-      gst = sqrt_(gs2);
-      const R g2 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
-      grad[0][0] = (gs2 - g2) / (gst + ut[0]) * a.inv_h;      // (u*^tau - u^tau)/h without cancellation
-      grad[0][1] = (sx - ut[1]) * a.inv_h; grad[0][2] = (sy - ut[2]) * a.inv_h; grad[0][3] = (sn_ - ut[3]) * a.inv_h;
-      gdiv = gst;
+      up3[0] = up[0]; up3[1] = up[sf]; up3[2] = up[2 * sf];
     } else {
       gst = a.gstar[cg];
-      const R g12 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
-      const R gn2 = R(1) + un_[1] * un_[1] + un_[2] * un_[2] + un_[3] * un_[3];
-      grad[0][0] = (g12 - gn2) / (ut[0] + un_[0]) * a.inv_h;
-      grad[0][1] = (ut[1] - un_[1]) * a.inv_h; grad[0][2] = (ut[2] - un_[2]) * a.inv_h;
-      grad[0][3] = (ut[3] - un_[3]) * a.inv_h;
-      gdiv = ut[0];
     }
-    if (a.milne) {
-      grad[3][0] += ut[3] * a.inv_tau;    // Eq.25
-      grad[3][3] += ut[0] * a.inv_tau;    // Eq.26
-    }
-    const R T_c = eos_T(a.eos, e_c);
-    is_source(ut, grad, pic, e_c, P_c, T_c, a.inv_5etas_hbarc, a.milne != 0, a.inv_tau, S + 4);
   }
 
-  const R w_n = e_n + P_n;
-  R QTn[4];
-  QTn[0] = a.tf_n * (w_n * un_[0] * un_[0] - P_n + pin[0]);
-  QTn[1] = a.tf_n * (w_n * un_[0] * un_[1] + pin[1]);
-  QTn[2] = a.tf_n * (w_n * un_[0] * un_[2] + pin[2]);
-  QTn[3] = a.tf_n * (w_n * un_[0] * un_[3] + pin[3]);
-
-  R pnew[10], M[4];
-  const R ig = R(1) / gdiv;
-  if (MODE != 2) {
-#pragma unroll
-    for (int m = 0; m < 10; ++m) pnew[m] = USE_PI ? (un_[0] * pin[m] + a.h * S[4 + m]) * ig : R(0);    // Eq.49
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) M[mu] = (QTn[mu] + a.h * S[mu]) * a.inv_tf_1 - pnew[mu];              // Eq.50-51
-  } else {
-#pragma unroll
-    for (int m = 0; m < 10; ++m)
-      pnew[m] = USE_PI ? R(0.5) * (un_[0] * pin[m] + gst * pic[m] + a.h * S[4 + m]) * ig : R(0);         // Eq.52
-    R QT1[4];
-    QT1[0] = a.tf_1 * (w_c * ut[0] * ut[0] - P_c + pic[0]);
-    QT1[1] = a.tf_1 * (w_c * ut[0] * ut[1] + pic[1]);
-    QT1[2] = a.tf_1 * (w_c * ut[0] * ut[2] + pic[2]);
-    QT1[3] = a.tf_1 * (w_c * ut[0] * ut[3] + pic[3]);
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) M[mu] = R(0.5) * (QTn[mu] + QT1[mu] + a.h * S[mu]) * a.inv_tf_1 - pnew[mu];  // Eq.53-54
-  }
-
-  // ---- root-find (Eq.51/54), warp-uniform iteration count --------------------------------------------
+  // ---- sources, stage update, root-find, limiter (hydro_stage_update.cuh) -------------------------
   unsigned flags = 0;
-  R e_new, P_new, cs2_new, ux_new, uy_new, un_new, g_new;
-  rootfind_warp(a.eos, M[0], M[1], M[2], M[3], e_c, a.root_iters, a.e_floor, a.v_max, e_new, P_new, cs2_new, ux_new,
-                uy_new, un_new, g_new, flags);
-  if (USE_PI) limit_pi_P(a.xi, e_new, P_new, pnew, flags);
+  Cell<R> nw;
+  R cs2_new;
+  stage_update<R, VISC, MODE>(a, S, cc, cn_, grad, up3, gst, nw, cs2_new, flags);
+  const R* ut = cc.u;
+  const R e_new = nw.e, P_new = nw.P, ux_new = nw.u[1], uy_new = nw.u[2], un_new = nw.u[3], g_new = nw.u[0];
+  const R* pnew = nw.pi;
 
   // ---- write state + extended slots ----------------------------------------------------------------
   if (active) {

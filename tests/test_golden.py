@@ -20,7 +20,7 @@ def test_oracle_reproduces_golden():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("kernel", [1, 2, 3])
 def test_cuda_matches_golden(crossover, kernel):
     from paper_1802_04449_b200 import Hydro
     c = make_golden.CASE
