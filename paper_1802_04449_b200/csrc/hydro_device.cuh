@@ -50,6 +50,46 @@ template <> __device__ __forceinline__ float rsqrt_<float>(float x) { return 1.0
 template <typename R> __device__ __forceinline__ R sqrt_(R x);
 template <> __device__ __forceinline__ double sqrt_<double>(double x) { return sqrt(x); }
 template <> __device__ __forceinline__ float sqrt_<float>(float x) { return sqrtf(x); }
+// Fast reciprocal / square roots for the production kernels (kernel 1 keeps the IEEE forms above): hardware seed plus
+// Newton steps, no slow path.  fp64: rcp.approx / rsqrt.approx give ~20 bits, two Newton steps reach <= 2 ulp (the
+// IEEE division and sqrt cost 25-30 instructions and a subroutine call each; ~15 of them sit on the per-plane critical
+// path of the tile kernel).  fp32: the .approx instructions themselves (<= 2 ulp).
+__device__ __forceinline__ double frcp_(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ float frcp_(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ double frsqrt_(double x) {      // x > 0
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double h = 0.5 * y, e = fma(-(x * y), h, 0.5);
+  y = fma(y, e, y);
+  h = 0.5 * y; e = fma(-(x * y), h, 0.5);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ float frsqrt_(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ double fsqrt_(double x) {       // x >= 0
+  const double y = frsqrt_(x > 0.0 ? x : 1.0);
+  const double s = x * y;
+  return fma(fma(-s, s, x), 0.5 * y, s);                   // one correction step on s = x rsqrt(x)
+}
+__device__ __forceinline__ float fsqrt_(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 template <typename R> __device__ __forceinline__ R abs_(R x) { return x < R(0) ? -x : x; }
 template <typename R> __device__ __forceinline__ R max_(R a, R b) { return a > b ? a : b; }
 template <typename R> __device__ __forceinline__ R min_(R a, R b) { return a < b ? a : b; }

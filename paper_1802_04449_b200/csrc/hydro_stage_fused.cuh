@@ -67,15 +67,15 @@ __device__ __forceinline__ R kt_div2(const R q[5], const R f[5], R cl, R cr, R t
 // signal speeds of one cell along the three axes from u~ (A6); cs2 from the EoS at the cell
 template <typename R>
 __device__ __forceinline__ void signal_speeds3(R g, R ux, R uy, R un, R cs2, R& cx, R& cy, R& cn) {
-  const R ig = R(1) / g;
+  const R ig = frcp_(g);
   const R ig2 = ig * ig;                                  // 1 - v^2 = 1/gamma^2
   const R v2 = (ux * ux + uy * uy + un * un) * ig2;
-  const R cs = sqrt_(cs2), omc = R(1) - cs2;
-  const R D = R(1) / (R(1) - v2 * cs2), base = R(1) - v2 * cs2, csg = cs * ig;
+  const R cs = fsqrt_(cs2), omc = R(1) - cs2;
+  const R D = frcp_(R(1) - v2 * cs2), base = R(1) - v2 * cs2, csg = cs * ig;
   const R vx = ux * ig, vy = uy * ig, vn = un * ig;
-  cx = (fabs_(vx) * omc + csg * sqrt_(max_(base - vx * vx * omc, R(0)))) * D;
-  cy = (fabs_(vy) * omc + csg * sqrt_(max_(base - vy * vy * omc, R(0)))) * D;
-  cn = (fabs_(vn) * omc + csg * sqrt_(max_(base - vn * vn * omc, R(0)))) * D;
+  cx = (fabs_(vx) * omc + csg * fsqrt_(max_(base - vx * vx * omc, R(0)))) * D;
+  cy = (fabs_(vy) * omc + csg * fsqrt_(max_(base - vy * vy * omc, R(0)))) * D;
+  cn = (fabs_(vn) * omc + csg * fsqrt_(max_(base - vn * vn * omc, R(0)))) * D;
 }
 
 #ifndef CLV_MINB

@@ -139,7 +139,7 @@ __device__ __forceinline__ void qf(const R* __restrict__ pt, const PtAux<R>& x, 
     Q = x.wg * umu; Fl = x.wua * umu;
     if (f == 0) Q -= x.P;
     if (f == AX + 1) Fl += x.P;
-    if (USE_PI) { Q += pt[(4 + f) * FST]; Fl += pt[(4 + c_pidx[AX + 1][f]) * FST]; }
+    if (USE_PI) { Q += pt[(4 + f) * FST]; Fl += pt[(4 + pidx_f(AX + 1, f)) * FST]; }
   } else {
     const R v = pt[f * FST];
     Q = x.g * v; Fl = x.ua * v;
@@ -256,7 +256,7 @@ template <typename R>
 __device__ __forceinline__ void derive(const EosDev<R>& eos, const R* __restrict__ pt, R& e, R& ux, R& uy, R& un, R& g,
                                        R& P, R& cs2) {
   e = pt[0]; ux = pt[FST]; uy = pt[2 * FST]; un = pt[3 * FST];
-  g = sqrt_(R(1) + ux * ux + uy * uy + un * un);
+  g = fsqrt_(R(1) + ux * ux + uy * uy + un * un);
   eos_P(eos, e, P, cs2);
 }
 
@@ -273,7 +273,7 @@ __device__ __forceinline__ int ghost_list(int i, int n, int periodic, int out[4]
 
 // =====================================================================================================================
 template <typename R, bool VISC, int MODE>
-__global__ void __launch_bounds__(TILE_THREADS, 1)
+__global__ void __launch_bounds__(TILE_THREADS, (sizeof(R) == 4 ? 2 : 1))
 stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap) {
   constexpr bool USE_PI = VISC && (MODE != 0);
   constexpr int NFS = USE_PI ? 14 : 4;          // evolved fields whose fluxes are formed
@@ -448,6 +448,20 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
         gyp = sm.yaux[0][row + HALO + 1][lane]; Pyp = sm.yaux[1][row + HALO + 1][lane]; cyp = sm.yaux[2][row + HALO + 1][lane];
         __syncthreads();
       }
+      // the tail of this plane reads the cell's state n (stage 2) or history (stage 1) from global memory: start those
+      // lines moving towards L1 now, behind the flux trips
+      const int ic = active ? i : 0, jc = active ? j : 0;
+      const long long cell = (long long)(k + HALO) * a.pz + (long long)(jc + HALO) * a.py + (ic + HALO);
+      if (centre && (lane & 15) == 0) {      // one request per 128-byte line of the row
+        if (MODE == 2) {
+#pragma unroll
+          for (int f = 0; f < (VISC ? 14 : 4); ++f) asm volatile("prefetch.global.L1 [%0];" ::"l"(a.sn + cell + f * a.pf));
+          if (USE_PI) asm volatile("prefetch.global.L1 [%0];" ::"l"(a.gstar + cell));
+        } else if (MODE == 1 && USE_PI) {
+#pragma unroll
+          for (int f = 0; f < 3; ++f) asm volatile("prefetch.global.L1 [%0];" ::"l"(a.uprev + cell + f * a.pf));
+        }
+      }
       // point quantities of the three stencils (eta: planes p, p-1, p-2; x: i-1, i, i+1; y: j-1, j, j+1)
       const PtAux<R> zp = pt_aux(e_p, hp.g, un_p, hp.P);
       const PtAux<R> z1 = pt_aux(r1[0], h1.g, r1[3 * FST], h1.P);
@@ -531,8 +545,8 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
           phase_b(is_t_tag, fa + 1, t, 1, Sb, QLb, FLb, QRb, FRb);
         }
       };
-#pragma unroll 1
-      for (int t = 0; t < 2; ++t) trip(std::true_type{}, t);
+#pragma unroll
+      for (int t = 0; t < 2; ++t) trip(std::true_type{}, t);      // unrolled: the T-field index is a constant
       if (USE_PI) {
 #pragma unroll 1
         for (int t = 2; t < NTRIP; ++t) trip(std::false_type{}, t);
@@ -573,14 +587,12 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
           mbar_expect_tx(&sm.bar[s2], STAGE_BYTES);
           tma_load_plane(&sm.ring[s2][0][0][0], &tmap, &sm.bar[s2], X0, Y0, p + 1 + HALO);
         }
-        const int ic = active ? i : 0, jc = active ? j : 0;
-        const long long cell = (long long)(k + HALO) * a.pz + (long long)(jc + HALO) * a.py + (ic + HALO);
         if (MODE == 2) {
           const R* __restrict__ sn = a.sn + cell;
           cn_.e = sn[0]; cn_.u[1] = sn[a.pf]; cn_.u[2] = sn[2 * a.pf]; cn_.u[3] = sn[3 * a.pf];
 #pragma unroll
           for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(4 + m) * a.pf] : R(0);
-          cn_.u[0] = sqrt_(R(1) + cn_.u[1] * cn_.u[1] + cn_.u[2] * cn_.u[2] + cn_.u[3] * cn_.u[3]);
+          cn_.u[0] = fsqrt_(R(1) + cn_.u[1] * cn_.u[1] + cn_.u[2] * cn_.u[2] + cn_.u[3] * cn_.u[3]);
           R cs2n;
           eos_P(a.eos, cn_.e, cn_.P, cs2n);
         }

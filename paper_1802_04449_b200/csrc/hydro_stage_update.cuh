@@ -42,30 +42,30 @@ __device__ __forceinline__ void rootfind_warp(const EosDev<R>& eos, R M0, R Mx, 
   R M2 = Mx * Mx + My * My + Mn * Mn;
   const R lim = v_max * M0;
   if (M2 > lim * lim) {
-    const R sc = lim * rsqrt_(M2);
+    const R sc = lim * frsqrt_(M2);
     Mx *= sc; My *= sc; Mn *= sc; M2 = lim * lim; flags |= 2u;
   }
   R e, P, cs2;
   if (eos.kind == 0) {
     const R d = M0 * M0 - M2;
-    e = R(3) * d / (M0 + sqrt_(M0 * M0 + R(3) * d));
+    e = R(3) * d * frcp_(M0 + fsqrt_(M0 * M0 + R(3) * d));
     P = e * R(1.0 / 3.0); cs2 = R(1.0 / 3.0);
   } else {
     const R tol = (sizeof(R) == 8) ? R(1e-15) : R(2e-7);
     const R tol2 = (sizeof(R) == 8) ? R(1e-9) : R(1e-4);
     R lo = R(0), hi = M0;
     e = e_start;
-    if (!(e > lo && e < hi)) e = M0 - M2 / (M0 + M0 * R(1.0 / 3.0));
+    if (!(e > lo && e < hi)) e = M0 - M2 * frcp_(M0 + M0 * R(1.0 / 3.0));
     if (!(e > lo && e < hi)) e = R(0.5) * M0;
     for (int it = 0; it < iters; ++it) {
       eos_P(eos, e, P, cs2);
-      const R inv = R(1) / (M0 + P);
+      const R inv = frcp_(M0 + P);
       const R g = M0 - M2 * inv - e;
       const bool conv = !(abs_(g) > tol * M0);
       if (__all_sync(0xffffffffu, conv)) break;
       const R dg = M2 * cs2 * inv * inv - R(1);
       if (g > R(0)) lo = e; else hi = e;
-      R en = e - g / dg;
+      R en = e - g * frcp_(dg);
       if (!(en >= lo && en <= hi)) en = R(0.5) * (lo + hi);
       e = conv ? e : en;
       // Newton converges quadratically on the (piecewise linear, convex) g: a step taken from a residual
@@ -73,7 +73,7 @@ __device__ __forceinline__ void rootfind_warp(const EosDev<R>& eos, R M0, R Mx, 
       if (__all_sync(0xffffffffu, !(abs_(g) > tol2 * M0))) break;
     }
     eos_P(eos, e, P, cs2);
-    const R g = M0 - M2 / (M0 + P) - e;
+    const R g = M0 - M2 * frcp_(M0 + P) - e;
     if (abs_(g) > R(1e3) * tol * M0) flags |= 4u;
   }
   if (vac) e = R(0);
@@ -81,13 +81,13 @@ __device__ __forceinline__ void rootfind_warp(const EosDev<R>& eos, R M0, R Mx, 
     e = e_floor; flags |= 1u;
     eos_P(eos, e, P, cs2);
   }
-  const R iw = R(1) / (M0 + P);
+  const R iw = frcp_(M0 + P);
   const R vx = Mx * iw, vy = My * iw, vn = Mn * iw;
-  const R gam = rsqrt_(R(1) - (vx * vx + vy * vy + vn * vn));
+  const R gam = frsqrt_(R(1) - (vx * vx + vy * vy + vn * vn));
   ux = gam * vx; uy = gam * vy; un = gam * vn;
   e_out = e; P_out = P; cs2_out = cs2;
   // u~^tau consistent with the stored u~^i (what a consumer would recompute): sqrt(1 + u.u)
-  g_out = sqrt_(R(1) + ux * ux + uy * uy + un * un);
+  g_out = fsqrt_(R(1) + ux * ux + uy * uy + un * un);
 }
 
 // pi limiter (A14) with P(e) supplied
@@ -99,7 +99,7 @@ __device__ __forceinline__ void limit_pi_P(R xi, R e, R P, R pi[10], unsigned& f
   const R mag2 = abs_(pp);
   const R lim2 = xi * xi * (e * e + R(3) * P * P);
   if (mag2 > lim2) {
-    const R r = sqrt_(lim2) * rsqrt_(mag2);
+    const R r = fsqrt_(lim2 * frcp_(mag2));
 #pragma unroll
     for (int m = 0; m < 10; ++m) pi[m] *= r;
     flags |= 16u;
@@ -126,15 +126,15 @@ __device__ __forceinline__ void stage_update(const A& a, R S[14], const Cell<R>&
     if (MODE == 1) {
       const R sx = R(2) * ut[1] - up[0], sy = R(2) * ut[2] - up[1], sn_ = R(2) * ut[3] - up[2];
       const R gs2 = R(1) + sx * sx + sy * sy + sn_ * sn_;
-      gst = sqrt_(gs2);
+      gst = fsqrt_(gs2);
       const R g2 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
-      grad[0][0] = (gs2 - g2) / (gst + ut[0]) * a.inv_h;      // (u*^tau - u^tau)/h without cancellation
+      grad[0][0] = (gs2 - g2) * frcp_(gst + ut[0]) * a.inv_h;      // (u*^tau - u^tau)/h without cancellation
       grad[0][1] = (sx - ut[1]) * a.inv_h; grad[0][2] = (sy - ut[2]) * a.inv_h; grad[0][3] = (sn_ - ut[3]) * a.inv_h;
       gdiv = gst;
     } else {
       const R g12 = R(1) + ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3];
       const R gn2 = R(1) + sn.u[1] * sn.u[1] + sn.u[2] * sn.u[2] + sn.u[3] * sn.u[3];
-      grad[0][0] = (g12 - gn2) / (ut[0] + sn.u[0]) * a.inv_h;
+      grad[0][0] = (g12 - gn2) * frcp_(ut[0] + sn.u[0]) * a.inv_h;
       grad[0][1] = (ut[1] - sn.u[1]) * a.inv_h; grad[0][2] = (ut[2] - sn.u[2]) * a.inv_h;
       grad[0][3] = (ut[3] - sn.u[3]) * a.inv_h;
       gdiv = ut[0];
@@ -156,7 +156,7 @@ __device__ __forceinline__ void stage_update(const A& a, R S[14], const Cell<R>&
   QTn[3] = a.tf_n * (w_n * sn.u[0] * sn.u[3] + (USE_PI ? sn.pi[3] : R(0)));
 
   R M[4];
-  const R ig = R(1) / gdiv;
+  const R ig = frcp_(gdiv);
   if (MODE != 2) {
 #pragma unroll
     for (int m = 0; m < 10; ++m) o.pi[m] = USE_PI ? (sn.u[0] * sn.pi[m] + a.h * S[4 + m]) * ig : R(0);   // Eq.49

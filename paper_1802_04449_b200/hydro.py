@@ -15,7 +15,7 @@ from . import build as _build
 
 HYDRO_MEM_DEVICE, HYDRO_MEM_HOST = 0, 1
 SYMBOLS = ["hydro_workspace_bytes", "hydro_create", "hydro_load", "hydro_set_history", "hydro_read_history",
-           "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_destroy", "hydro_strerror"]
+           "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_kernel", "hydro_destroy", "hydro_strerror"]
 
 
 class hydro_grid(Structure):
@@ -69,6 +69,8 @@ def load_library():
     lib.hydro_diag.argtypes = [c_void_p, POINTER(hydro_diag_t)]
     lib.hydro_launch_count.restype = c_longlong
     lib.hydro_launch_count.argtypes = [c_void_p]
+    lib.hydro_kernel.restype = c_int
+    lib.hydro_kernel.argtypes = [c_void_p]
     lib.hydro_destroy.restype = None
     lib.hydro_destroy.argtypes = [c_void_p]
     lib.hydro_strerror.restype = ctypes.c_char_p
@@ -220,6 +222,10 @@ class Hydro:
 
     def launch_count(self) -> int:
         return int(self._lib.hydro_launch_count(self._h))
+
+    def kernel(self) -> int:
+        """The stage kernel in use (1 reference, 2 per-cell fused, 3 tile); kernel=0 resolves by precision."""
+        return int(self._lib.hydro_kernel(self._h))
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:

@@ -20,27 +20,32 @@ def test_full_size_first_steps(crossover, which, steps):
     o.load(T)
     o.step(steps)
     ref = o.read()
-    g = from_config(cfg, crossover)
-    g.load(T)
-    g.step(steps)
-    er = errors(crossover, ref, g.read())
-    print(which, "fp64", er, g.diag())
-    assert er["rel_e"] <= 1e-10 * (1 if steps == 1 else 10) and er["rel_T"] <= 1e-10 * (1 if steps == 1 else 10)
-    assert er["rel_pi"] <= 1e-9 and er["l2_e"] <= 1e-13 and er["l2_T"] <= 1e-12
-    do, dg = o.diag(), g.diag()
-    assert np.allclose(dg["cfl"], do["cfl"], rtol=1e-9) and abs(dg["e_max"] / do["e_max"] - 1) < 1e-10
-    assert dg["nan"] == 0 and dg["root_unconverged"] == 0
-    del g
-    g32 = from_config(cfg, crossover, precision=32)
-    g32.load(T.astype(np.float32))
-    g32.step(steps)
-    er = errors(crossover, ref, g32.read())
-    print(which, "fp32", er)
-    assert er["l2_e"] <= 2e-4 and er["l2_T"] <= 2e-4 and g32.diag()["nan"] == 0
+    do = o.diag()
+    for kernel in (2, 3):                       # both production kernels, fp64
+        g = from_config(cfg, crossover, kernel=kernel)
+        g.load(T)
+        g.step(steps)
+        er = errors(crossover, ref, g.read())
+        print(which, "fp64 kernel", kernel, er, g.diag())
+        assert er["rel_e"] <= 1e-10 * (1 if steps == 1 else 10) and er["rel_T"] <= 1e-10 * (1 if steps == 1 else 10)
+        assert er["rel_pi"] <= 1e-9 and er["l2_e"] <= 1e-13 and er["l2_T"] <= 1e-12
+        dg = g.diag()
+        assert np.allclose(dg["cfl"], do["cfl"], rtol=1e-9) and abs(dg["e_max"] / do["e_max"] - 1) < 1e-10
+        assert dg["nan"] == 0 and dg["root_unconverged"] == 0
+        del g
+    for kernel in (2, 3):
+        g32 = from_config(cfg, crossover, precision=32, kernel=kernel)
+        g32.load(T.astype(np.float32))
+        g32.step(steps)
+        er = errors(crossover, ref, g32.read())
+        print(which, "fp32 kernel", kernel, er)
+        assert er["l2_e"] <= 2e-4 and er["l2_T"] <= 2e-4 and g32.diag()["nan"] == 0
+        del g32
 
 
+@pytest.mark.parametrize("kernel", [2, 3])
 @pytest.mark.parametrize("eta_s", [0.0, 0.2])
-def test_gubser_on_gpu(conformal, eta_s):
+def test_gubser_on_gpu(conformal, eta_s, kernel):
     """configs[1]b at the stated resolution (201x201x1, dx = 0.05) from tau = 1 to 1.5 on the GPU, against the
     Gubser solution (closed form for eta/s = 0, IS ODE for 0.2)."""
     from analytic_refs import Gubser
@@ -52,7 +57,7 @@ def test_gubser_on_gpu(conformal, eta_s):
     gub = Gubser(1.0, eta_s)
     h = dx / 10
     T, pi = gub.T_tau_mu(1.0, X, Y)
-    g = Hydro(n, n, 1, dx, dx, 1.0, h, 1.0, conformal, eta_s, pi_limit_xi=0.0, minmod_theta=2.0)
+    g = Hydro(n, n, 1, dx, dx, 1.0, h, 1.0, conformal, eta_s, pi_limit_xi=0.0, minmod_theta=2.0, kernel=kernel)
     g.load(np.ascontiguousarray(T), np.ascontiguousarray(pi) if eta_s > 0 else None)
     g.set_history(np.ascontiguousarray(gub.fields(1.0 - h, X, Y)[1][1:]))
     g.step(int(round((t1 - 1.0) / h)))

@@ -205,3 +205,50 @@ def test_tile_exact_and_tiny_grids(crossover, kernel, shape, bc):
     o32.step(3); g32.step(3)
     er = errors(crossover, o32.read(), g32.read())
     assert er["l2_e"] <= 2e-4 and er["l2_T"] <= 2e-4 and er["rel_e"] < 1e-3
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_limiter_fires_in_many_cells(crossover, kernel):
+    """Row a8 exercised for real: pi of the order of e, so that the limiter (A14) acts in well over
+    10 % of the cells in both stages; one step at the 1e-10 bar, event counts equal."""
+    nx, ny, nz = 40, 20, 12
+    e, v, pi = inputs.ic_random_smooth(nx, ny, nz, seed=21, vmax=0.4)
+    pi[4:] *= 35.0                                   # spatial components up to ~e: beyond xi sqrt(e^2 + 3P^2) in many cells
+    from parity_util import pressure
+    P = pressure(crossover, e)
+    g2 = 1.0 / (1.0 - (v ** 2).sum(0))
+    T = np.stack([(e + P) * g2 - P, (e + P) * g2 * v[0], (e + P) * g2 * v[1], (e + P) * g2 * v[2]]) + pi[:4]
+    cfg = inputs.Config("lim", nx, ny, nz, 0.2, 0.2, 0.2, 0.8, 0.02, 1, 0.16, "crossover", bc=(0, 1, 0))
+    o, g = run_pair(cfg, crossover, T, pi, 0, gkw=dict(kernel=kernel))
+    o.step(1); g.step(1)
+    er = errors(crossover, o.read(), g.read())
+    do, dg = o.diag(), g.diag()
+    print("limiter case", er, do, dg)
+    assert do["pi_limited"] > 0.2 * cfg.cells                     # counted over both stages
+    assert dg["pi_limited"] == do["pi_limited"] and dg["clamped"] == do["clamped"] and dg["floored"] == do["floored"]
+    assert er["rel_e"] <= 1e-10 and er["rel_T"] <= 1e-10 and er["rel_pi"] <= 1e-10
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_vacuum_corner_floor(crossover, kernel):
+    """Row a9 / A8: a vacuum corner (T^{tau tau} below the floor) next to matter: the floor fires there, the acausal
+    clamp fires on the rim that the matter pushes into the vacuum; one step, counts equal."""
+    nx, ny, nz = 36, 18, 10
+    e, v, pi = inputs.ic_random_smooth(nx, ny, nz, seed=22, vmax=0.3, with_pi=False)
+    from parity_util import pressure
+    P = pressure(crossover, e)
+    g2 = 1.0 / (1.0 - (v ** 2).sum(0))
+    T = np.stack([(e + P) * g2 - P, (e + P) * g2 * v[0], (e + P) * g2 * v[1], (e + P) * g2 * v[2]])
+    T[:, :5, :9, :14] = 0.0
+    T[0, :5, :9, :14] = 1e-9                          # below e_floor = 1e-7
+    cfg = inputs.Config("vac", nx, ny, nz, 0.2, 0.2, 0.2, 0.8, 0.02, 1, 0.08, "crossover", bc=(0, 0, 1))
+    o, g = run_pair(cfg, crossover, T, None, 0, gkw=dict(kernel=kernel))
+    d0 = o.diag()
+    assert d0["floored"] >= 5 * 9 * 14
+    o.step(1); g.step(1)
+    er = errors(crossover, o.read(), g.read())
+    do, dg = o.diag(), g.diag()
+    print("vacuum corner", er, do, dg)
+    assert do["floored"] > d0["floored"]                           # the floor also fires during the step
+    assert dg["floored"] == do["floored"] and dg["clamped"] == do["clamped"] and dg["pi_limited"] == do["pi_limited"]
+    assert er["rel_e"] <= 1e-10 and er["rel_T"] <= 1e-10 and er["rel_pi"] <= 1e-10
