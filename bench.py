@@ -1,18 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused viscous KT-RK2 step (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--precision 64|32] [--kernel 0|1|2]
-    python bench.py --impl reference ...      # the CPU oracle, timed as it stands (bounded sample)
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--precision 64|32] [--kernel 0|1|2|3]
+    python bench.py --impl reference ...      # the CPU oracle, timed as it stands (bounded sample per step)
 
 A "step" is one full RK2 step (both stages: KT fluxes of T^{tau mu} and pi^{mu nu} on three axes, Milne and
 Israel-Stewart sources, root-find, pi limiter, reductions) over the whole grid.  Workload = BASELINE.json
 configs[4]: 301x301x201 cells, dx=dy=0.1, deta=0.08, tau0=0.4, dtau=0.01, eta/s=0.16, crossover EoS table,
-8000 seeded partons with momentum (synthetic stand-in for AMPT events).  Prints ONE JSON line.
+8000 seeded partons with momentum (synthetic stand-in for AMPT events).  Prints ONE JSON line: the headline is
+the fp64 run (BASELINE.json's metric names fp64 and fp32; the fp32 run of the same grid and step count is the
+"fp32" sub-record of the same line).
 
 Timing: W >= 3 warm-up steps, then exactly K steps between CUDA events recorded on the stream the
 kernels are launched on, stream-synchronised on both sides (barrier + max over ranks for N > 1).  The
-working set (3 x 14 fields x 146 MB) is far larger than the 126 MB L2, so no flush is needed.
-N > 1: one process per GPU, each evolving its own seeded event (replicas, no data-path collective).
+working set (3 state buffers of 14-19 fields x 146 MB) is far larger than the 126 MB L2, so no flush is needed.
+N > 1: one process per GPU, each evolving its own seeded event (replicas, no data-path collective);
+`--gpus N` without a torchrun environment re-executes itself under torch.distributed.run.
 """
 from __future__ import annotations
 
@@ -33,7 +36,8 @@ from paper_1802_04449_b200 import inputs  # noqa: E402
 
 METRIC = "viscous KT-RK2 cell-updates/s at 301x301x201"
 UNIT = "cell-updates/s"
-ALGO_BYTES_PER_CELL_STEP = {64: 584, 32: 292}     # 73 words per cell per RK2 step
+ALGO_WORDS = {True: 73, False: 20}     # compulsory words per cell per RK2 step (viscous / ideal)
+NSM, ISSUE_PER_SM = 148, 4             # B200: SMs, warp-instruction issue slots per clock per SM (4 schedulers)
 
 
 def measured_hbm_peak():
@@ -44,33 +48,51 @@ def measured_hbm_peak():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_counters():
+    """Per-launch counters of the stage kernels taken from the committed ncu captures (profiles/round2_counters.json):
+    dram bytes and executed warp instructions, keyed f<precision>_k<kernel>."""
+    p = os.path.join(ROOT, "profiles", "round2_counters.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f)
+    return {}
+
+
 class ClockSampler(threading.Thread):
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    """SM clock / throttle reasons during the run: one long-lived `nvidia-smi -lms 50` (B200_PROFILING.md recipe),
+    started before the warm-up; every line is stamped when it is read."""
 
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index=0):
+    def __init__(self, index=0, period_ms=50):
         super().__init__(daemon=True)
-        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", str(period_ms)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
+        except Exception:
+            self.proc = None
 
     def run(self):
-        while not self._stop_evt.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
-                if out.returncode == 0 and out.stdout.strip():
-                    self.rows.append([time.perf_counter()] + [c.strip() for c in out.stdout.strip().split(",")])
-            except Exception:
-                pass
-            self._stop_evt.wait(0.2)
+        if not self.proc:
+            return
+        for line in self.proc.stdout:
+            self.rows.append([time.perf_counter()] + [c.strip() for c in line.strip().split(",")])
 
-    def stop(self, t0=None, t1=None):
-        self._stop_evt.set()
-        self.join(timeout=10)
+    def stop(self, windows):
+        """windows: list of (t0, t1) perf_counter intervals of the timed regions."""
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+        self.join(timeout=5)
+        inside = [r[1:] for r in self.rows if any(t0 <= r[0] <= t1 for t0, t1 in windows)]
         sm, reasons, mx = [], set(), None
-        inside = [r[1:] for r in self.rows if t0 is not None and t0 <= r[0] <= t1]
         for r in (inside or [r[1:] for r in self.rows]):
             try:
                 sm.append(float(r[0])); mx = float(r[1])
@@ -80,7 +102,7 @@ class ClockSampler(threading.Thread):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm), "samples_inside_timed_region": len(inside)}
+                "samples": len(self.rows), "samples_inside_timed_region": len(inside), "period_ms": 50}
 
 
 def sub_config(nx, ny, nz, partons):
@@ -90,42 +112,69 @@ def sub_config(nx, ny, nz, partons):
     return c
 
 
-def cpu_oracle_rate(nx, ny, nz, steps):
-    """Times the oracle as it stands on the host cores; returns (cell-updates/s, threads, description)."""
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
+def make_oracle(nx, ny, nz):
     from oracle import Oracle
-    partons = max(8, int(round(8000 * nx * ny * nz / (301.0 * 301 * 201))))
+    full = (nx, ny, nz) == (301, 301, 201)
+    partons = 8000 if full else max(8, int(round(8000 * nx * ny * nz / (301.0 * 301 * 201))))
     cfg = sub_config(nx, ny, nz, partons)
     eos = inputs.crossover_table()
     T, _ = inputs.ic_partons(cfg, inputs.seed_for(4))
     o = Oracle(cfg.nx, cfg.ny, cfg.nz, cfg.dx, cfg.dy, cfg.deta, cfg.dtau, cfg.tau0, eos, cfg.eta_over_s)
     o.load(T)
-    t0 = time.perf_counter()
-    o.step(steps)
-    dt = time.perf_counter() - t0
-    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    sample = (f"{nx}x{ny}x{nz} sub-box of configs[4] (same spacings, EoS table, eta/s=0.16, sampler at the same "
-              f"parton density: {partons} partons), {steps} RK2 step(s), {dt:.1f} s wall")
-    return cfg.cells * steps / dt, threads, sample, dt
+    what = ("configs[4] itself (301x301x201, 8000 partons)" if full else
+            f"{nx}x{ny}x{nz} sub-box of configs[4] (same spacings, EoS table, eta/s=0.16, sampler at the same parton "
+            f"density: {partons} partons)")
+    return o, cfg, what
+
+
+def omp_threads():
+    return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    """--impl reference: the oracle as it stands on the host cores.  Every step of the run is one RK2 step of a bounded
+    sample (a 96x96x64 sub-box of configs[4]); W warm-up steps, then exactly K timed steps."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
-    nx, ny, nz = 96, 96, 64
-    for _ in range(max(args.warmup, 0) and 1):
-        cpu_oracle_rate(32, 32, 16, 1)
-    rate, threads, sample, dt = cpu_oracle_rate(nx, ny, nz, max(1, min(args.steps, 4)))
+    o, cfg, what = make_oracle(96, 96, 64)
+    o.step(max(args.warmup, 0))
+    t0 = time.perf_counter()
+    o.step(args.steps)
+    dt = time.perf_counter() - t0
+    rate = cfg.cells * args.steps / dt
+    sample = f"{what}; {args.steps} RK2 steps after {args.warmup} warm-up steps, {dt:.1f} s wall"
     line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, min(args.steps, 4)),
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[4] 301x301x201 viscous eta/s=0.16 crossover EoS; oracle timed on a bounded "
-                                   "sample of it", "sample": sample},
-            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "config": {"workload": "configs[4] 301x301x201 viscous eta/s=0.16 crossover EoS; the oracle is timed on a "
+                                   "bounded sample of it per step", "sample": sample, "cells_per_step": cfg.cells},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": omp_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+def roofline_record(cells, precision, viscous, ms_total, launches, kernel, counters, clocks):
+    """The dominant kernel is the stage kernel (two launches per step, 100 % of hydro_step)."""
+    peak, peak_src = measured_hbm_peak()
+    algo_per_launch = ALGO_WORDS[viscous] * (precision // 8) * cells / 2.0
+    avg_launch_s = ms_total * 1e-3 / launches
+    achieved = algo_per_launch / avg_launch_s / 1e9
+    c = counters.get(f"f{precision}_k{kernel}", {}) if viscous else {}
+    rec = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "traffic": c.get("dram_bytes_per_launch"), "peak_source": peak_src,
+           "kernel": {1: "stage_ref_kernel", 2: "stage_fused_kernel", 3: "stage_tile_kernel"}[kernel] +
+                     " (average of the stage-1 and stage-2 launches)",
+           "algorithmic_bytes_per_launch": algo_per_launch, "avg_launch_ms": avg_launch_s * 1e3}
+    # second view: what actually limits the kernel is instruction issue / fp64 latency, not HBM (DESIGN.md section 5).
+    # Measured warp instructions per launch (ncu, profiles/) over the issue slots available during the measured launch.
+    wi = c.get("warp_inst_per_launch")
+    if wi:
+        sm_hz = 1e6 * ((clocks or {}).get("sm_mhz") or 1965.0)
+        rec["issue"] = {"bound": "alu", "achieved": wi / avg_launch_s, "peak": NSM * ISSUE_PER_SM * sm_hz,
+                        "unit": "warp-inst/s", "frac": wi / avg_launch_s / (NSM * ISSUE_PER_SM * sm_hz),
+                        "source": c.get("source")}
+    return rec
 
 
 def main():
@@ -133,17 +182,26 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--precision", type=int, default=64, choices=(64, 32))
+    ap.add_argument("--precision", type=int, default=64, choices=(64, 32),
+                    help="precision of the headline run (default 64; the other precision is the sub-record)")
     ap.add_argument("--kernel", type=int, default=0)
     ap.add_argument("--impl", default="b200", choices=("b200", "reference"))
     ap.add_argument("--grid", default="301,301,201", help="nx,ny,nz (default = configs[4])")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-steps", type=int, default=3, help="oracle steps of configs[4] for cpu_baseline (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-second-precision", action="store_true")
     ap.add_argument("--eta-over-s", type=float, default=0.16,
                     help="context runs only (0 = the ideal-fluid path, PAPER.md Table II); the headline is 0.16")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # launched by hand without torchrun: start one rank per GPU ourselves
+        port = str(29500 + os.getpid() % 2000)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", port, os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     args.warmup = max(args.warmup, 3)
 
     import torch
@@ -166,13 +224,8 @@ def main():
         cfg.extra["partons"] = max(8, int(round(8000 * cfg.cells / (301.0 * 301 * 201))))
     eos = inputs.crossover_table()
     T, _ = inputs.ic_partons(cfg, replicas.rank_seed(4, rank))     # one seeded event per rank
-    npdt = np.float64 if args.precision == 64 else np.float32
-    tdt = torch.float64 if args.precision == 64 else torch.float32
-
-    h = from_config(cfg, eos, precision=args.precision, kernel=args.kernel, device=f"cuda:{local}")
-    T_dev = torch.from_numpy(T.astype(npdt)).to(dev)
-    h.load(T_dev)
-    stream = h.stream
+    viscous = args.eta_over_s > 0
+    counters = ncu_counters()
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -180,28 +233,37 @@ def main():
             dist.barrier()
             torch.cuda.synchronize(dev)
 
-    # ---- device-resident timing ----------------------------------------------------------------
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start()
-    h.step(args.warmup)
-    barrier()
-    l0 = h.launch_count()
-    tw0 = time.perf_counter()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(stream)
-    h.step(args.steps)
-    ev1.record(stream)
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    launches = h.launch_count() - l0
-    clocks = sampler.stop(tw0, time.perf_counter()) if sampler else None
-    d = h.diag()
-    value, ms = replicas.aggregate_rate(cfg.cells, args.steps, ms, world, dev)
-    ms_per_step = ms / args.steps
+    windows = []
+
+    def timed_run(precision):
+        """Device-resident timing of K steps in one precision; returns the context and the record."""
+        npdt = np.float64 if precision == 64 else np.float32
+        h = from_config(cfg, eos, precision=precision, kernel=args.kernel, device=f"cuda:{local}")
+        h.load(torch.from_numpy(T.astype(npdt)).to(dev))
+        h.step(args.warmup)
+        barrier()
+        l0 = h.launch_count()
+        tw0 = time.perf_counter()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(h.stream)
+        h.step(args.steps)
+        ev1.record(h.stream)
+        barrier()
+        windows.append((tw0, time.perf_counter()))
+        ms_local = ev0.elapsed_time(ev1)
+        launches = h.launch_count() - l0
+        value, ms = replicas.aggregate_rate(cfg.cells, args.steps, ms_local, world, dev)
+        return h, dict(value=value, ms=ms, launches=int(launches), kernel=h.kernel(), diag=h.diag())
+
+    h, main_rec = timed_run(args.precision)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): load -> step -> read, every step ------
     N = cfg.cells
+    npdt = np.float64 if args.precision == 64 else np.float32
+    tdt = torch.float64 if args.precision == 64 else torch.float32
     T_host = torch.from_numpy(T.astype(npdt)).pin_memory()
     e_h = torch.empty((nz, ny, nx), dtype=tdt, pin_memory=True)
     u_h = torch.empty((4, nz, ny, nx), dtype=tdt, pin_memory=True)
@@ -211,62 +273,74 @@ def main():
         h.step(1)
         h.read(out=(e_h, u_h, None))      # the method's result: e and u^mu
 
+    e2e = None
     if args.e2e_steps > 0:
         e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.e2e_steps):
-        e2e_step()
-    barrier()
-    e2e_s = max(time.perf_counter() - t0, 1e-9)
-    e2e_s = replicas.max_over_ranks(e2e_s, dev)
-    esz = 8 if args.precision == 64 else 4
-    e2e = {"value": world * N * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz,
-           "d2h_bytes_per_step": 5 * N * esz, "steps": args.e2e_steps,
-           "what": "hydro_load(host T^{tau mu}) + hydro_step(1) + hydro_read(host e, u^mu) per step, pinned buffers"}
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        barrier()
+        e2e_s = replicas.max_over_ranks(max(time.perf_counter() - t0, 1e-9), dev)
+        esz = 8 if args.precision == 64 else 4
+        e2e = {"value": world * N * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * N * esz,
+               "d2h_bytes_per_step": 5 * N * esz, "steps": args.e2e_steps,
+               "what": "hydro_load(host T^{tau mu}) + hydro_step(1) + hydro_read(host e, u^mu) per step, pinned buffers; "
+                       "pi^{mu nu} is neither loaded (initial pi = 0, as in configs[4]) nor read back: a viscous restart "
+                       "would copy 10 more words per cell each way"}
+    del h
 
+    # ---- the other precision of BASELINE.json's metric, same grid and step count -------------------------
+    second = None
+    if not args.no_second_precision:
+        p2 = 32 if args.precision == 64 else 64
+        h2, second = timed_run(p2)
+        second["precision"] = p2
+        del h2
+
+    clocks = sampler.stop(windows) if sampler else None
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the fused stage kernel: 2 launches per step) ------------------
-    peak, peak_src = measured_hbm_peak()
-    words = 73 if args.eta_over_s > 0 else 20            # compulsory words per cell per RK2 step
-    algo_per_launch = words * (args.precision // 8) * cfg.cells / 2.0
-    avg_launch_s = ms * 1e-3 / launches
-    achieved = algo_per_launch / avg_launch_s / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        with open(tp) as f:
-            traffic = json.load(f).get(f"f{args.precision}_k{h_kernel_name(args.kernel)}")
-    # second view: the same launch against the plain fp64 (fp32) pipe, 3 400 arithmetic
-    # instructions per cell per stage on 148 SMs x 64 (128) lanes at the SM clock sampled during the run
-    lanes = 64 if args.precision == 64 else 128
-    sm_hz = 1e6 * ((clocks or {}).get("sm_mhz") or 1965.0)
-    alu_frac = (3400.0 * cfg.cells / avg_launch_s) / (148 * lanes * sm_hz)
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "alu_frac": alu_frac,
-                "traffic": traffic, "peak_source": peak_src, "kernel": "fused RK2 stage kernel (avg of stage 1 and 2)",
-                "algorithmic_bytes_per_launch": algo_per_launch, "avg_launch_ms": avg_launch_s * 1e3}
+    roofline = roofline_record(cfg.cells, args.precision, viscous, main_rec["ms"], main_rec["launches"],
+                               main_rec["kernel"], counters, clocks)
+    second_rec = None
+    if second:
+        p2 = second["precision"]
+        second_rec = {"dtype": f"f{p2}", "value": second["value"], "unit": UNIT, "steps": args.steps,
+                      "ms_per_step": second["ms"] / args.steps, "kernel": second["kernel"],
+                      "gpu_launches": second["launches"],
+                      "roofline": roofline_record(cfg.cells, p2, viscous, second["ms"], second["launches"],
+                                                  second["kernel"], counters, clocks),
+                      "diag": {k: second["diag"][k] for k in ("tau", "step", "e_max", "nan", "root_unconverged")}}
 
     cpu = None
-    if not args.no_cpu_baseline and world == 1:      # rank 0 at N = 1 only
-        rate, threads, sample, _ = cpu_oracle_rate(96, 96, 64, 2)
-        cpu = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+    if not args.no_cpu_baseline and world == 1 and args.cpu_steps > 0:      # rank 0 at N = 1 only
+        full = (nx, ny, nz) == (301, 301, 201)
+        o, ocfg, what = make_oracle(nx, ny, nz) if full else make_oracle(96, 96, 64)
+        t0 = time.perf_counter()
+        o.step(args.cpu_steps)
+        dt = time.perf_counter() - t0
+        cpu = {"value": ocfg.cells * args.cpu_steps / dt, "unit": UNIT, "cores": omp_threads(), "kind": "oracle",
+               "sample": f"{what}, {args.cpu_steps} RK2 steps, {dt:.1f} s wall (load and bootstrap not timed)"}
+        del o
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
+    d = main_rec["diag"]
+    line = {"metric": METRIC, "value": main_rec["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main_rec["ms"] / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
+            "data": "synthetic",
             "config": {"workload": f"configs[4]: {nx}x{ny}x{nz} cells, dx=dy=0.1 fm, deta=0.08, tau0=0.4, dtau=0.01, "
                                    f"eta/s={args.eta_over_s:g}, crossover EoS table (2000 nodes), {cfg.extra['partons']} seeded "
                                    "partons with momentum, outflow boundaries",
-                       "cells": cfg.cells, "precision": args.precision, "kernel": args.kernel,
-                       "l2": "working set (3 x 14 fields) >> 126 MB L2, no flush needed",
+                       "cells": cfg.cells, "precision": args.precision, "kernel": main_rec["kernel"],
+                       "kernel_requested": args.kernel,
+                       "l2": "working set (3 state buffers) >> 126 MB L2, no flush needed",
                        "parallelism": "1 event per GPU (replicas)" if world > 1 else "1 GPU"},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
-            "clocks": clocks,
+            "roofline": roofline, "fp32" if args.precision == 64 else "fp64": second_rec,
+            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": main_rec["launches"], "clocks": clocks,
             "diag": {k: d[k] for k in ("tau", "step", "cfl", "e_max", "floored", "clamped", "pi_limited", "nan",
                                        "root_unconverged")},
             "context": {"paper": "CLVisc: 16.9 M cell-updates/s viscous fp32 on AMD FirePro S9150 (Table II, "
@@ -274,10 +348,6 @@ def main():
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
-
-
-def h_kernel_name(k):
-    return {0: "default", 1: "ref", 2: "fused"}.get(k, str(k))
 
 
 if __name__ == "__main__":

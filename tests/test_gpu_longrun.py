@@ -36,9 +36,13 @@ def test_full_length_stability(crossover, which, precision, kernel):
         assert np.isfinite(d["e_max"])
     print(which, precision, "e_max", ["%.4g" % v for v in emax], d)
     assert d["step"] == cfg.steps
-    # Bjorken-like dilution: e_max falls monotonically once the first chunk is over
-    assert all(b <= a * (1 + 1e-6) for a, b in zip(emax[1:], emax[2:])), emax
-    assert emax[-1] < 0.5 * emax[0]
+    # Bjorken-like dilution: e_max falls monotonically once the first chunk is over -- down to the scale of the isolated
+    # rim spikes.  On the clamped rim single dilute cells jump to e ~ 0.3-0.6 GeV/fm^3 for a few steps in EVERY
+    # implementation, the oracle included (measured on the 96x96x64 sub-box: at step 125 the oracle holds a cell at 0.51
+    # where its own FMA-contracted build and both CUDA kernels hold 0.03-0.06; test_moving_event_drift_is_rounding_chaos),
+    # so once the core has diluted below ~1 GeV/fm^3 the maximum may sit on such a cell.
+    assert all(b <= max(a * (1 + 1e-6), 1.0) for a, b in zip(emax[1:], emax[2:])), emax
+    assert emax[-1] < 0.5 * emax[0] and max(emax[2:]) <= emax[1]
     e, u, p = g.read()
     assert np.isfinite(e).all() and np.isfinite(u).all() and np.isfinite(p).all()
     assert e.min() >= 1e-7 * (1 - 1e-6) and u[0].max() <= 22.4 * (1 + 1e-3)       # floor (A8) and v_max clamp (A7)
