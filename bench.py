@@ -101,8 +101,11 @@ class ClockSampler(threading.Thread):
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
+        ts = [r[0] for r in self.rows]
+        period = 1e3 * float(np.median(np.diff(ts))) if len(ts) > 2 else None     # what nvidia-smi really delivered
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(self.rows), "samples_inside_timed_region": len(inside), "period_ms": 50}
+                "samples": len(self.rows), "samples_inside_timed_region": len(inside), "period_ms_requested": 50,
+                "period_ms_measured": period}
 
 
 def sub_config(nx, ny, nz, partons):

@@ -85,6 +85,11 @@ typedef struct {
   void *stream;
   void *workspace;
   size_t workspace_bytes;
+  /* SURVEY 8(f)-2 (PAPER.md:58-60 Eq.4, :169 Eq.33, :412-437): the lambda_1 term  -(lambda_1/tau_pi) pi^{<mu}_l pi^{nu>l}
+   * with lambda_1 = lambda1_hat / e, 0 = off (the paper's production setting); and the coefficient of
+   * the relaxation time tau_pi = tau_pi_coeff eta_v/(T s), <= 0 selects the paper's 5.  The paper's
+   * closed-form Gubser test uses lambda1_hat = -10 and tau_pi_coeff = 4 lambda1_hat^2 / 9. */
+  double lambda1_hat, tau_pi_coeff;
 } hydro_opts;
 
 /* Diagnostics (PAPER.md:640 for e_max).  cfl[a] = max over cells of

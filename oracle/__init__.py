@@ -168,7 +168,7 @@ class Oracle:
         acted = self._lib.oracle_limit_pi(self._h, float(e), _p(p))
         return p, bool(acted)
 
-    OPT_HEUN_PRINTED = 0
+    OPT_HEUN_PRINTED, OPT_LAMBDA1_HAT, OPT_C_TAU = 0, 1, 2
 
     def set_option(self, key, value):
         if self._lib.oracle_set_option(self._h, int(key), float(value)):

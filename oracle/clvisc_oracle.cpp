@@ -97,6 +97,11 @@ struct Oracle {
   double theta = 1.1, e_floor = 1e-7, xi = 1.0, v_max = 1.0 - 1e-10;
   int strict_eq53 = 0;
   int heun_printed = 0;   // A26: 0 = Shu-Osher bookkeeping (default), 1 = Eq.52-53 exactly as printed
+  // the lambda_1 term of Eq.4 / Eq.33 and a free relaxation-time coefficient,
+  //   tau_pi = c_tau eta_v/(T s)   (paper: c_tau = 5),   lambda_1 = lambda1_hat / e
+  // needed by the paper's closed-form Gubser test (L = 2, eta_v/s = 0.2, lambda1_hat = -10 and
+  // tau_pi from eta_hat lambda1_hat^2 = 3 tau_pi_hat, i.e. c_tau = 4 lambda1_hat^2 / 9).
+  double lambda1_hat = 0.0, c_tau = 5.0;
   int step = 0;
   bool loaded = false;
   size_t N;
@@ -263,9 +268,33 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
       for (int m = 0; m < 4; ++m) Du[n] += ut[m] * grad[m][n];              // D~ = u~^lambda nabla~_lambda
     }
     double e = s.e[c], P = pt.P[c], T = pt.T[c];
-    double inv_taupi = T / (5.0 * o.eta_s * HBARC);     // tau_pi = 5 eta_v/(T s)
-    double etav_over_taupi = (e + P) / 5.0;             // eta_v/tau_pi = (e+P)/5
+    double inv_taupi = T / (o.c_tau * o.eta_s * HBARC);     // tau_pi = 5 eta_v/(T s)
+    double etav_over_taupi = (e + P) / o.c_tau;             // eta_v/tau_pi = (e+P)/5
     auto pic = [&](int m, int n) { return s.pi[PIDX[m][n]][c]; };
+    // lambda_1 term (Eq.33): -(lambda_1/tau_pi) pi~^{<mu}_lambda pi~^{nu>lambda}, with the projector
+    // of Eq.5 written out: X^{ab} = pi~^{a l} g~_{l k} pi~^{k b};  X^{<mn>} = Delta^{mn}_{ab} X^{ab},
+    // Delta^{mn ab} = 1/2 (Delta^{ma} Delta^{nb} + Delta^{mb} Delta^{na}) - 1/3 Delta^{mn} Delta^{ab}.
+    double PP[4][4] = {{0}};
+    if (o.lambda1_hat != 0.0) {
+      double X[4][4], Dl[4][4];   // Dl = Delta^{ab} = g~^{ab} - u~^a u~^b
+      for (int a = 0; a < 4; ++a)
+        for (int b = 0; b < 4; ++b) {
+          X[a][b] = 0.0;
+          for (int l = 0; l < 4; ++l) X[a][b] += pic(a, l) * GMET[l] * pic(l, b);
+          Dl[a][b] = (a == b ? GMET[a] : 0.0) - ut[a] * ut[b];
+        }
+      for (int m = 0; m < 4; ++m)
+        for (int n = 0; n < 4; ++n) {
+          double acc = 0.0;
+          for (int a = 0; a < 4; ++a)
+            for (int b = 0; b < 4; ++b) {
+              // indices of X lowered with g~: X_{ab} = g_aa g_bb X^{ab}
+              double Xl = GMET[a] * GMET[b] * X[a][b];
+              acc += (0.5 * (Dl[m][a] * Dl[n][b] + Dl[m][b] * Dl[n][a]) - Dl[m][n] * Dl[a][b] / 3.0) * Xl;
+            }
+          PP[m][n] = acc;
+        }
+    }
     for (int m = 0; m < 4; ++m)
       for (int n = m; n < 4; ++n) {
         // sigma~^{mu nu}: expansion of Eq.5
@@ -273,6 +302,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
                      - (2.0 / 3.0) * ((m == n ? GMET[m] : 0.0) - ut[m] * ut[n]) * theta_exp;
         double p = pic(m, n);
         double src = -p * inv_taupi + etav_over_taupi * sig - p * theta_exp / 3.0;
+        if (o.lambda1_hat != 0.0) src -= (o.lambda1_hat / e) * inv_taupi * PP[m][n];
         double contr = 0.0;
         for (int b = 0; b < 4; ++b) contr += (ut[m] * pic(n, b) + ut[n] * pic(m, b)) * GMET[b] * Du[b];
         src -= contr;
@@ -637,10 +667,12 @@ int oracle_limit_pi(void* h, double e, double* pi10) {
 }
 
 // Options that are not part of oracle_create's argument list.  key 0: heun_printed (A26; 0 default, 1 = Eq.52-53
-// as printed).  Returns 0, or -1 for an unknown key.
+// as printed); key 1: lambda1_hat; key 2: c_tau.  Returns 0, or -1 for an unknown key / bad value.
 int oracle_set_option(void* h, int key, double value) {
   Oracle& o = *static_cast<Oracle*>(h);
   if (key == 0) { o.heun_printed = value != 0.0 ? 1 : 0; return 0; }
+  if (key == 1) { o.lambda1_hat = value; return 0; }
+  if (key == 2) { if (!(value > 0.0)) return -1; o.c_tau = value; return 0; }
   return -1;
 }
 

@@ -275,7 +275,7 @@ struct hydro_ctx {
   hydro_grid grid;
   double dtau, tau0, eta_s;
   int precision, visc, kernel;
-  double theta, e_floor, xi, v_max;
+  double theta, e_floor, xi, v_max, lambda1_hat, c_tau;
   int root_iters;
   Layout L;
   char* ws;
@@ -361,7 +361,8 @@ TileArgs<R> tile_args(const hydro_ctx* c, double tau_rhs, double tau_n, double t
   a.scale[0] = (R)(1.0 / c->grid.dx); a.scale[1] = (R)(1.0 / c->grid.dy);
   a.scale[2] = (R)(milne ? 1.0 / (tau_rhs * c->grid.deta) : 1.0 / c->grid.deta);
   a.theta = (R)c->theta; a.e_floor = (R)c->e_floor; a.xi = (R)c->xi; a.v_max = (R)c->v_max;
-  a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (5.0 * c->eta_s * kHbarc) : 0.0);
+  a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (c->c_tau * c->eta_s * kHbarc) : 0.0);
+  a.inv_ctau = (R)(1.0 / c->c_tau); a.lam1 = (R)c->lambda1_hat;
   a.root_iters = c->root_iters;
   a.eos = eos_of<R>(c);
   a.diag = c->diag;
@@ -450,7 +451,8 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
   a.scale[0] = (R)(1.0 / c->grid.dx); a.scale[1] = (R)(1.0 / c->grid.dy);
   a.scale[2] = (R)(milne ? 1.0 / (tau_rhs * c->grid.deta) : 1.0 / c->grid.deta);
   a.theta = (R)c->theta; a.e_floor = (R)c->e_floor; a.xi = (R)c->xi; a.v_max = (R)c->v_max;
-  a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (5.0 * c->eta_s * kHbarc) : 0.0);
+  a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (c->c_tau * c->eta_s * kHbarc) : 0.0);
+  a.inv_ctau = (R)(1.0 / c->c_tau); a.lam1 = (R)c->lambda1_hat;
   a.root_iters = c->root_iters;
   a.eos = eos_of<R>(c);
   a.diag = c->diag;
@@ -692,6 +694,8 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
   c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;
+  c->lambda1_hat = opts->lambda1_hat;
+  c->c_tau = opts->tau_pi_coeff > 0.0 ? opts->tau_pi_coeff : 5.0;
   c->L = L;
   c->ws = static_cast<char*>(opts->workspace);
   for (int b = 0; b < 3; ++b) c->buf[b] = c->ws + L.off_buf[b];

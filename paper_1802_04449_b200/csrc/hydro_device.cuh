@@ -171,22 +171,24 @@ __device__ __forceinline__ R kt_div(const R q[5], const R f[5], R cl, R cr, R th
 }
 
 // ---------------------------------------------------------------------------------------------
-// Israel-Stewart source (Eq.33 with lambda_i = 0), tilde components.
+// Israel-Stewart source (Eq.33 with lambda_2 = lambda_3 = 0), tilde components.
+//   tau_pi = c_tau eta_v/(T s)  (paper: c_tau = 5; inv_ctau = 1/c_tau),  lambda_1 = lam1_hat / e
 //   ut[4]      u~^mu at the cell
 //   grad[m][n] nabla~_m u~^n  (Eq.22, 24-26 already added by the caller)
 //   pi[10], e, P, T; out S[10] += source
 // ---------------------------------------------------------------------------------------------
 template <typename R>
 __device__ __forceinline__ void is_source(const R ut[4], const R grad[4][4], const R pi[10], R e, R P, R T,
-                                          R inv_5etas_hbarc, bool milne, R inv_tau, R S[10]) {
+                                          R inv_5etas_hbarc, bool milne, R inv_tau, R S[10], R inv_ctau = R(0.2),
+                                          R lam1_hat = R(0)) {
   const R gm[4] = {R(1), R(-1), R(-1), R(-1)};
   const R theta_exp = grad[0][0] + grad[1][1] + grad[2][2] + grad[3][3];
   R Du[4];
 #pragma unroll
   for (int n = 0; n < 4; ++n)
     Du[n] = ut[0] * grad[0][n] + ut[1] * grad[1][n] + ut[2] * grad[2][n] + ut[3] * grad[3][n];
-  const R inv_taupi = T * inv_5etas_hbarc;      // 1/tau_pi = T s/(5 eta_v)
-  const R eta_over_taupi = (e + P) * R(0.2);    // eta_v/tau_pi = (e+P)/5
+  const R inv_taupi = T * inv_5etas_hbarc;      // 1/tau_pi = T s/(c_tau eta_v)  (c_tau = 5)
+  const R eta_over_taupi = (e + P) * inv_ctau;  // eta_v/tau_pi = (e+P)/c_tau
   const int IDX[4][4] = {{0, 1, 2, 3}, {1, 4, 5, 6}, {2, 5, 7, 8}, {3, 6, 8, 9}};
   R w[4];
 #pragma unroll
@@ -213,6 +215,37 @@ __device__ __forceinline__ void is_source(const R ut[4], const R grad[4][4], con
       }
       S[IDX[m][n]] += src;
     }
+  // lambda_1 term (Eq.4 / Eq.33): -(lambda_1/tau_pi) pi~^{<mu}_lambda pi~^{nu>lambda}.
+  // X^{ab} = pi^{a l} g_{l k} pi^{k b};  Delta X Delta = X - u w^T - w u^T + u u^T s  with  w^a = X^{ab} u_b,
+  // s = u_a X^{ab} u_b;  the traceless part subtracts 1/3 Delta^{mn} (g_{ab} X^{ab} - s).
+  if (lam1_hat != R(0)) {
+    R X[4][4], wv[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = a; b < 4; ++b) {
+        X[a][b] = pi[IDX[a][0]] * pi[IDX[0][b]] - pi[IDX[a][1]] * pi[IDX[1][b]] - pi[IDX[a][2]] * pi[IDX[2][b]] -
+                  pi[IDX[a][3]] * pi[IDX[3][b]];
+        X[b][a] = X[a][b];
+      }
+    R sx = R(0), tr = R(0);
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      wv[a] = X[a][0] * ut[0] - X[a][1] * ut[1] - X[a][2] * ut[2] - X[a][3] * ut[3];
+      tr += gm[a] * X[a][a];
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a) sx += gm[a] * ut[a] * wv[a];
+    const R coef = lam1_hat / e * inv_taupi, third = (tr - sx) * R(1.0 / 3.0);
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int n = m; n < 4; ++n) {
+        const R proj = X[m][n] - ut[m] * wv[n] - wv[m] * ut[n] + ut[m] * ut[n] * sx -
+                       ((m == n ? gm[m] : R(0)) - ut[m] * ut[n]) * third;
+        S[IDX[m][n]] -= coef * proj;
+      }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -29,7 +29,8 @@ struct StageArgs {
   R h, inv_h;
   R scale[3];            // 1/dx, 1/dy, 1/(tau deta)  (Eq.40)
   R theta, e_floor, xi, v_max;
-  R inv_5etas_hbarc;     // 1/(5 (eta_v/s) hbarc)
+  R inv_5etas_hbarc;     // 1/(c_tau (eta_v/s) hbarc), c_tau = 5 unless set (tau_pi = c_tau eta_v/(T s))
+  R inv_ctau, lam1;      // 1/c_tau; lambda1_hat (lambda_1 = lambda1_hat / e)
   int root_iters;
   const R* in;           // state whose 13-point star is read
   const R* sn;           // MODE 2: state n (cell centre only)
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(256) stage_ref_kernel(const StageArgs<R> a) {
       grad[3][3] += ut[0] * a.inv_tau;    // Eq.26
     }
     const R T_c = eos_T(a.eos, e_c);
-    is_source(ut, grad, pic, e_c, P_c, T_c, a.inv_5etas_hbarc, a.milne != 0, a.inv_tau, S + 4);
+    is_source(ut, grad, pic, e_c, P_c, T_c, a.inv_5etas_hbarc, a.milne != 0, a.inv_tau, S + 4, a.inv_ctau, a.lam1);
   }
 
   // Q_T^n = tf_n T_f^{tau mu}(state n)

@@ -56,7 +56,7 @@ struct TileArgs {
   int milne;
   R tau, inv_tau, tf_n, tf_1, inv_tf_1, h, inv_h;
   R scale[3];
-  R theta, e_floor, xi, v_max, inv_5etas_hbarc;
+  R theta, e_floor, xi, v_max, inv_5etas_hbarc, inv_ctau, lam1;
   int root_iters;
   const R* sn;       // MODE 2: state n (centre only)
   const R* uprev;    // MODE 1: u~^i at n-1 (3 fields, stride pf)

@@ -21,7 +21,7 @@ struct Cell {
 };
 
 // A: any argument struct with the members milne, inv_tau, tf_n, tf_1, inv_tf_1, h, inv_h, xi, e_floor, v_max,
-// root_iters, inv_5etas_hbarc, eos.
+// root_iters, inv_5etas_hbarc, inv_ctau, lam1, eos.
 //   S[14]      in: S_KT (T fields 0..3, pi fields 4..13); clobbered
 //   c          the state the RHS was evaluated on (n in MODE 0/1, ' in MODE 2)
 //   n          state n at the cell (MODE 2; ignored otherwise)
@@ -144,7 +144,7 @@ __device__ __forceinline__ void stage_update(const A& a, R S[14], const Cell<R>&
       grad[3][3] += ut[0] * a.inv_tau;    // Eq.26
     }
     const R T_c = eos_T(a.eos, c.e);
-    is_source(ut, grad, c.pi, c.e, c.P, T_c, a.inv_5etas_hbarc, a.milne != 0, a.inv_tau, S + 4);
+    is_source(ut, grad, c.pi, c.e, c.P, T_c, a.inv_5etas_hbarc, a.milne != 0, a.inv_tau, S + 4, a.inv_ctau, a.lam1);
   }
 
   // Q_T^n = tf_n T_f^{tau mu}(state n)

@@ -124,6 +124,24 @@ def boost_tilde(u, pi, delta):
     return un, pin
 
 
+class GubserLambda1(Gubser):
+    """The paper's own closed-form second-order Gubser solution (Eq.72-76): with the lambda_1 term of
+    Eq.4 and  eta_hat lambda1_hat^2 = 3 tau_pi_hat,
+        e_hat ~ cosh(rho)^-(8/3 - 2/lambda1_hat),   pi_hat^{eta eta} = (2/lambda1_hat) e_hat  (C = -2A = -2B),
+    and the velocity of the ideal solution (fixed by the conformal map).  In the notation of Gubser above:
+    T_hat = T_hat0 cosh(rho)^-(2/3 - 1/(2 lambda1_hat)),  pibar = pi_hat^{eta eta}/(T_hat s_hat) = 3/(2 lambda1_hat).
+    With tau_pi = c_tau eta_v/(T s) the constraint reads c_tau = 4 lambda1_hat^2 / 9  (derivation: DESIGN.md A27)."""
+
+    def __init__(self, q=0.5, lambda1_hat=-10.0, That0=1.2):
+        self.q, self.eta_s, self.That0, self.lam = q, 0.2, That0, lambda1_hat
+        self.c_tau = 4.0 * lambda1_hat ** 2 / 9.0
+
+    def hat(self, rho):
+        rho = np.asarray(rho, dtype=np.float64)
+        Th = self.That0 * np.cosh(rho) ** (-(2.0 / 3.0 - 1.0 / (2.0 * self.lam)))
+        return Th, np.full_like(rho, 3.0 / (2.0 * self.lam))
+
+
 class ShiftedGubser:
     """SURVEY 8c pin 5: the Gubser solution translated by (t0, z0) in the (t, z) plane.  Poincare invariance
     makes it an exact solution of the same equations; seen from the unshifted Milne frame it has u~^eta != 0,

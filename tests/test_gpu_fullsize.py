@@ -75,3 +75,28 @@ def test_gubser_on_gpu(conformal, eta_s, kernel):
     if eta_s > 0:
         assert out["pixx"] < 0.012 and out["pinn"] < 0.01
         assert np.all(np.abs(p[[3, 6, 8]]) < 1e-12) and np.all(np.abs(u[3]) < 1e-12)
+
+
+@pytest.mark.parametrize("kernel", [1, 2, 3])
+def test_gubser_lambda1_on_gpu(conformal, kernel):
+    """SURVEY 8(f)-2 on the GPU: the lambda_1 term and the free tau_pi coefficient against the paper's closed-form
+    Gubser solution and against the oracle on the same grid."""
+    from oracle import Oracle
+    from paper_1802_04449_b200 import Hydro
+    from test_oracle_gubser import gubser_lambda1_run
+
+    def make_gpu(n, dx, h, lam, c_tau):
+        return Hydro(n, n, 1, dx, dx, 1.0, h, 1.0, conformal, 0.2, pi_limit_xi=0.0, minmod_theta=2.0, kernel=kernel,
+                     lambda1_hat=lam, tau_pi_coeff=c_tau)
+
+    def make_cpu(n, dx, h, lam, c_tau):
+        o = Oracle(n, n, 1, dx, dx, 1.0, h, 1.0, conformal, 0.2, pi_limit_xi=0.0, minmod_theta=2.0)
+        o.set_option(Oracle.OPT_LAMBDA1_HAT, lam); o.set_option(Oracle.OPT_C_TAU, c_tau)
+        return o
+    f, ratio, got = gubser_lambda1_run(make_gpu, 0.1, 1.5)
+    print("gubser lambda1 on GPU, kernel", kernel, f, ratio)
+    assert f["e"] < 1.5e-3 and f["pixx"] < 1.5e-3 and f["pinn"] < 1.5e-3 and abs(ratio - 2.0) < 0.05
+    _, _, ref = gubser_lambda1_run(make_cpu, 0.1, 1.5)
+    er = errors(conformal, ref, got)
+    print("   vs oracle", er)
+    assert er["rel_e"] <= 1e-9 and er["rel_pi"] <= 1e-9 and er["l2_e"] <= 1e-12

@@ -113,3 +113,48 @@ def test_gubser_configs1b_to_tau4(conformal, eta_s, theta):
     assert all(got[t1]["vr"] < 0.01 for t1 in got) and got[1.5]["e"] < 0.01
     if eta_s > 0:
         assert got[1.5]["pinn"] < 0.01 and np.all(np.abs(p[[3, 6, 8]]) < 1e-12)
+
+
+def gubser_lambda1_run(make, dx, t1, L=8.0, lam_on=True):
+    """The paper's closed-form test: L = 2 (q = 1/2), eta_v/s = 0.2, lambda1_hat = -10,
+    tau_pi from eta_hat lambda1_hat^2 = 3 tau_pi_hat; tau0 = 1.  `make(n, dx, h, lam, c_tau)` builds the solver."""
+    from analytic_refs import GubserLambda1
+    g = GubserLambda1()
+    n = int(round(2 * L / dx)) + 1
+    x = (np.arange(n) - (n - 1) / 2) * dx
+    Y, X = np.meshgrid(x, x, indexing="ij")
+    X, Y = X[None], Y[None]
+    h = dx / 10
+    T, pi = g.T_tau_mu(1.0, X, Y)
+    o = make(n, dx, h, g.lam if lam_on else 0.0, g.c_tau)
+    o.load(np.ascontiguousarray(T), np.ascontiguousarray(pi))
+    o.set_history(np.ascontiguousarray(g.fields(1.0 - h, X, Y)[1][1:]))
+    o.step(int(round((t1 - 1.0) / h)))
+    e, u, p = o.read()
+    ea, ua, pa = g.fields(t1, X, Y)
+    m = ea > 1e-3 * ea.max()
+    l2 = lambda a, b: float(np.sqrt(((a - b)[m] ** 2).sum() / (b[m] ** 2).sum()))
+    vr, vra = np.sqrt(u[1] ** 2 + u[2] ** 2) / u[0], np.sqrt(ua[1] ** 2 + ua[2] ** 2) / ua[0]
+    # "-tau^2 pi^{eta eta} is roughly two times pi^{xx}" at the centre (PAPER.md:447)
+    c = n // 2
+    ratio = -p[9][0, c, c] / p[4][0, c, c]
+    return dict(e=l2(e, ea), vr=l2(vr, vra), pixx=l2(p[4], pa[4]), pinn=l2(p[9], pa[9])), ratio, (e, u, p)
+
+
+def test_gubser_lambda1_closed_form(conformal):
+    """the lambda_1 term of Eq.4/33 against the paper's own closed-form solution (Eq.72-76): a pin of the
+    viscous sector that needs no ODE solver.  Second order under refinement; and the SAME run without the lambda_1 term
+    misses the solution by 4 % in pi^{eta eta} (so the term is really exercised)."""
+    def make(n, dx, h, lam, c_tau):
+        o = Oracle(n, n, 1, dx, dx, 1.0, h, 1.0, conformal, 0.2, pi_limit_xi=0.0, minmod_theta=2.0)
+        o.set_option(Oracle.OPT_LAMBDA1_HAT, lam)
+        o.set_option(Oracle.OPT_C_TAU, c_tau)
+        return o
+    c, rc, _ = gubser_lambda1_run(make, 0.2, 1.5)
+    f, rf, _ = gubser_lambda1_run(make, 0.1, 1.5)
+    print("gubser lambda1", c, f, rc, rf)
+    assert f["e"] < 1.5e-3 and f["pixx"] < 1.5e-3 and f["pinn"] < 1.5e-3 and f["vr"] < 0.01      # measured 1.1e-3, 9.8e-4, 1.2e-3
+    assert c["e"] / f["e"] > 3.5 and c["pixx"] / f["pixx"] > 3.0 and c["pinn"] / f["pinn"] > 3.0
+    assert abs(rf - 2.0) < 0.05
+    off, _, _ = gubser_lambda1_run(make, 0.1, 1.5, lam_on=False)
+    assert off["pinn"] > 0.03
