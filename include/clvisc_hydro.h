@@ -72,11 +72,11 @@ typedef struct {
  * <= 0 selects the default 0.999 (gamma <= 22.4; A7 gives the evidence); root_iters: fixed Newton iteration
  * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
  * stream); workspace: DEVICE memory of at least hydro_workspace_bytes(), 256-byte aligned.
- * kernel: 0 = default (the faster one for the precision as measured on B200: 3 for precision 32, 2 for precision 64);
- * 3 = tile kernel (hydro_stage_tile.cuh): TMA-staged 32x8 tiles marching along eta_s, every
- * slope and face flux computed once, 14-word ghosted SoA state; 2 = per-cell fused kernel on the extended 19-word state
- * (hydro_stage_fused.cuh); 1 = per-cell reference kernel (re-derives P, u^tau, c_a at every stencil point).  Kernels 1
- * and 2 are kept as in-library cross-checks. */
+ * kernel: 0 = default (the faster one as measured on B200: 2 in both precisions);
+ * 2 = per-cell fused kernel on the extended 19-word state (hydro_stage_fused.cuh); 3 = tile kernel
+ * (hydro_stage_tile.cuh): TMA-staged 32x8 tiles marching along eta_s, every slope and face flux computed once, 14-word
+ * ghosted SoA state; 1 = per-cell reference kernel (re-derives P, u^tau, c_a at every stencil point).  All three give
+ * the same results to rounding and are covered by the parity tests. */
 typedef struct {
   int precision;
   double minmod_theta, e_floor, pi_limit_xi, v_max;

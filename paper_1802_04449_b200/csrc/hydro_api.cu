@@ -13,7 +13,7 @@
 // offset is a compile-time immediate and a cell's whole state lies in one 4.8 KB stretch of DRAM.
 // buf X (+gstar) doubles as the staging area for host-memory load/read between steps.
 //
-// Kernel 3 (the tile kernel, default) uses a different field store: plain SoA with two ghost layers per side,
+// Kernel 3 (the tile kernel) uses a different field store: plain SoA with two ghost layers per side,
 //   [field][nz+4][ny+4][pitch]   (pitch = nx+4 rounded up to 16 bytes), nf = 4 / 14 fields and nothing derived,
 // addressed by TMA tensor maps (one per buffer and box depth) that hydro_create encodes.
 #include "../../include/clvisc_hydro.h"
@@ -46,10 +46,10 @@ struct Layout {
   size_t off_diag, off_eos, off_buf[3], off_gstar, total;
 };
 
-// kernel 0 = the faster one for the precision as measured on B200 at 301x301x201 (round 2):
-// fp32 -> the tile kernel (8.35 vs 8.77 ms per step), fp64 -> the per-cell fused kernel (14.3 vs 15.9 ms: with 8 warps
-// per SM the tile kernel cannot hide the fp64 latencies)
-static int resolve_kernel(int kernel, int precision) { return kernel != 0 ? kernel : (precision == 32 ? 3 : 2); }
+// kernel 0 = the faster one as measured on B200 at 301x301x201 (round 2): the per-cell fused
+// kernel in both precisions (fp64 14.4 vs 15.7 ms per step; fp32 7.6 vs 8.0 once the FMNMX minmod and the packed f32x2
+// arithmetic are in: the tile kernel cannot hide its latencies with 8 (fp64) / 16 (fp32) warps per SM)
+static int resolve_kernel(int kernel, int precision) { (void)precision; return kernel != 0 ? kernel : 2; }
 
 static bool make_layout(const hydro_grid* g, int precision, double eta_s, int kernel, Layout* L) {
   if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;

@@ -6,7 +6,7 @@
 //   * EXTENDED STATE: the producing kernel appends P, u^tau and the three signal speeds c_x, c_y, c_eta
 //     of every cell to the state it writes (5 extra words), so the 13-point star is READ, never
 //     re-derived: no EoS lookup, sqrt or division per stencil point (kernel 1 re-derives them 15 times).
-//   * cheap generalised minmod: 2 compares + 3 arithmetic fp64 instructions, sign logic on the integer pipe.
+//   * cheap generalised minmod (hmm4): 4 fp64-pipe instructions + selects on the integer pipe; fp32: FMNMX clamp form.
 //   * the overall factor tau of Q_T, F_T (Eq.18) is applied once to the flux difference, not per point.
 //   * warp-uniform early exit of the Newton iteration (no intra-warp divergence).
 #pragma once
@@ -29,39 +29,91 @@ __device__ __forceinline__ float fabs_(float x) { return fabsf(x); }
 __device__ __forceinline__ double fmin_(double a, double b) { return fmin(a, b); }
 __device__ __forceinline__ float fmin_(float a, float b) { return fminf(a, b); }
 
-// hmm(dm, dp) = 1/2 minmod(theta dm, (dm+dp)/2, theta dp)
-//             = 1/2 sign(dm) min(theta min(|dm|,|dp|), |dm+dp|/2) when dm, dp share a sign, else 0.
-// Written so that ptxas emits 5 fp64 instructions (2 DSETP, DADD, 2 DMUL) + 1 DMUL for the signed 1/2 and 8
-// integer-pipe instructions; plain fmin() costs twice that (NaN quieting and register moves).
-__device__ __forceinline__ double hmm(double dm, double dp, double theta) {
+// hmm4(dm, dp) = 4 x the half slope = 2 minmod(theta dm, (dm+dp)/2, theta dp)
+//              = the smaller in magnitude of (2 theta s, dm + dp), s = the smaller in magnitude of (dm, dp), when dm and
+//                dp share a sign, else 0.  th2 = 2 theta.  The callers fold the factor 1/4 into an FMA.
+// fp64: both candidates carry the sign already, so there is no sign word to build: 5 fp64-pipe instructions (2 DSETP,
+// DADD, 2 DMUL) + 7 on the integer pipe (4 selects, xor, compare, select of the 1/0 factor); the round-1 form spent
+// 7 + 7 (profiles/round2_kernels.md).  fp32: clamp form on FMNMX / FMNMX3, 7 instructions and no integer logic.
+__device__ __forceinline__ double hmm4(double dm, double dp, double th2) {
+  const bool same = (__double2hiint(dm) ^ __double2hiint(dp)) >= 0;
   const double s = fabs(dm) < fabs(dp) ? dm : dp;
-  const double t = fabs(s) * theta;
-  const double h = fabs(dm + dp) * 0.5;
-  const double m = t < h ? t : h;
-  const int hm = __double2hiint(dm), hp = __double2hiint(dp);
-  int k;                                                      // high word of copysign(0.5, dm), one LOP3
-  asm("lop3.b32 %0, %1, 0x80000000, %2, 0xEA;" : "=r"(k) : "r"(hm), "r"(0x3fe00000));     // (a & b) | c
-  const int khi = ((hm ^ hp) >= 0) ? k : 0;                   // +-0.5 or 0
-  return m * __hiloint2double(khi, 0);
+  const double t = s * th2;
+  const double h = dm + dp;
+  const double m = fabs(t) < fabs(h) ? t : h;
+  // times 1 or 0: measured faster on B200 than zeroing with two selects (14.60 vs 14.78 ms per step) or zeroing s early
+  return m * __hiloint2double(same ? 0x3ff00000 : 0, 0);
 }
-__device__ __forceinline__ float hmm(float dm, float dp, float theta) {
-  const float m = fminf(theta * fminf(fabsf(dm), fabsf(dp)), 0.5f * fabsf(dm + dp));
-  const int hm = __float_as_int(dm), hp = __float_as_int(dp);
-  const int k = ((hm ^ hp) >= 0) ? (0x3f000000 | (hm & 0x80000000)) : 0;       // +-0.5f or 0
-  return m * __int_as_float(k);
+__device__ __forceinline__ float hmm4(float dm, float dp, float th2) {
+  // t = 2 theta min(|dm|, |dp|) when the signs agree, else 0:  max(min(dm,dp), -max(dm,dp), 0)
+  const float p = fminf(dm, dp), q = fmaxf(dm, dp);
+  float t0, r;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(t0) : "f"(p), "f"(-q), "f"(0.0f));
+  const float t = t0 * th2;
+  asm("min.f32 %0, %1, %2;" : "=f"(r) : "f"(fmaxf(dm + dp, -t)), "f"(t));      // clamp(dm + dp, -t, t)
+  return r;
 }
 
 // 2 (H_{i+1/2} - H_{i-1/2}) for one field (the factor 1/2 of Eq.41 is folded into the caller's scale)
 template <typename R>
-__device__ __forceinline__ R kt_div2(const R q[5], const R f[5], R cl, R cr, R theta) {
+__device__ __forceinline__ R kt_div2(const R q[5], const R f[5], R cl, R cr, R th2) {
   const R dq0 = q[1] - q[0], dq1 = q[2] - q[1], dq2 = q[3] - q[2], dq3 = q[4] - q[3];
   const R df0 = f[1] - f[0], df1 = f[2] - f[1], df2 = f[3] - f[2], df3 = f[4] - f[3];
-  const R hq1 = hmm(dq0, dq1, theta), hq2 = hmm(dq1, dq2, theta), hq3 = hmm(dq2, dq3, theta);
-  const R hf1 = hmm(df0, df1, theta), hf2 = hmm(df1, df2, theta), hf3 = hmm(df2, df3, theta);
-  // Hr - Hl with the f-part collected: (f3 + f2 - hf3 + hf2) - (f2 + f1 - hf2 + hf1) = (df1 + df2) - hf3 - hf1 + 2 hf2
-  const R fpart = ((df1 + df2) - (hf3 + hf1)) + R(2) * hf2;
-  const R qr = (dq2 - hq3) - hq2, ql = (dq1 - hq2) - hq1;
+  const R mq1 = hmm4(dq0, dq1, th2), mq2 = hmm4(dq1, dq2, th2), mq3 = hmm4(dq2, dq3, th2);
+  const R mf1 = hmm4(df0, df1, th2), mf2 = hmm4(df1, df2, th2), mf3 = hmm4(df2, df3, th2);
+  // Hr - Hl with the f-part collected (half slopes h = m/4):
+  //   (f3 + f2 - hf3 + hf2) - (f2 + f1 - hf2 + hf1) = (df1 + df2) - (hf3 + hf1) + 2 hf2
+  const R fpart = R(0.5) * mf2 + (R(-0.25) * (mf3 + mf1) + (df1 + df2));
+  const R qr = R(-0.25) * (mq3 + mq2) + dq2, ql = R(-0.25) * (mq2 + mq1) + dq1;
   return fpart - cr * qr + cl * ql;
+}
+
+// ---- packed fp32 pairs (sm_100a add/mul/fma.f32x2 -> FADD2 / FMUL2 / FFMA2): two fields per instruction -------------
+// The fp32 stage is bound by instruction issue (profiles/round2_kernels.md), so the arithmetic of the two fields of a
+// trip is issued as one packed instruction; min/max stay scalar (there is no packed FMNMX).
+#ifndef CLV_PACK32
+#define CLV_PACK32 1
+#endif
+struct F2 { float x, y; };
+__device__ __forceinline__ unsigned long long pk_(F2 a) {
+  unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y)); return r;
+}
+__device__ __forceinline__ F2 up_(unsigned long long r) {
+  F2 a; asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r)); return a;
+}
+__device__ __forceinline__ F2 bc2(float s) { F2 a = {s, s}; return a; }
+__device__ __forceinline__ F2 add2(F2 a, F2 b) {
+  unsigned long long r; asm("add.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b))); return up_(r);
+}
+__device__ __forceinline__ F2 sub2(F2 a, F2 b) { const F2 nb = {-b.x, -b.y}; return add2(a, nb); }
+__device__ __forceinline__ F2 mul2(F2 a, F2 b) {
+  unsigned long long r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b))); return up_(r);
+}
+__device__ __forceinline__ F2 fma2(F2 a, F2 b, F2 c) {
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b)), "l"(pk_(c)));
+  return up_(r);
+}
+__device__ __forceinline__ F2 hmm4_2(F2 dm, F2 dp, F2 th2) {
+  float t0x, t0y, rx, ry;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(t0x) : "f"(fminf(dm.x, dp.x)), "f"(-fmaxf(dm.x, dp.x)), "f"(0.0f));
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(t0y) : "f"(fminf(dm.y, dp.y)), "f"(-fmaxf(dm.y, dp.y)), "f"(0.0f));
+  const F2 t0 = {t0x, t0y};
+  const F2 t = mul2(t0, th2), s = add2(dm, dp);
+  asm("min.f32 %0, %1, %2;" : "=f"(rx) : "f"(fmaxf(s.x, -t.x)), "f"(t.x));
+  asm("min.f32 %0, %1, %2;" : "=f"(ry) : "f"(fmaxf(s.y, -t.y)), "f"(t.y));
+  const F2 r = {rx, ry};
+  return r;
+}
+// kt_div2 for a pair of fields
+__device__ __forceinline__ F2 kt_div2_2(const F2 q[5], const F2 f[5], F2 cl, F2 ncr, F2 th2) {
+  const F2 dq0 = sub2(q[1], q[0]), dq1 = sub2(q[2], q[1]), dq2 = sub2(q[3], q[2]), dq3 = sub2(q[4], q[3]);
+  const F2 df0 = sub2(f[1], f[0]), df1 = sub2(f[2], f[1]), df2 = sub2(f[3], f[2]), df3 = sub2(f[4], f[3]);
+  const F2 mq1 = hmm4_2(dq0, dq1, th2), mq2 = hmm4_2(dq1, dq2, th2), mq3 = hmm4_2(dq2, dq3, th2);
+  const F2 mf1 = hmm4_2(df0, df1, th2), mf2 = hmm4_2(df1, df2, th2), mf3 = hmm4_2(df2, df3, th2);
+  const F2 fpart = fma2(bc2(0.5f), mf2, fma2(bc2(-0.25f), add2(mf3, mf1), add2(df1, df2)));
+  const F2 qr = fma2(bc2(-0.25f), add2(mq3, mq2), dq2), ql = fma2(bc2(-0.25f), add2(mq2, mq1), dq1);
+  return fma2(cl, ql, fma2(ncr, qr, fpart));      // ncr = -cr
 }
 
 // signal speeds of one cell along the three axes from u~ (A6); cs2 from the EoS at the cell
@@ -78,6 +130,13 @@ __device__ __forceinline__ void signal_speeds3(R g, R ux, R uy, R un, R cs2, R& 
   cn = (fabs_(vn) * omc + csg * fsqrt_(max_(base - vn * vn * omc, R(0)))) * D;
 }
 
+#ifndef CLV_PFD
+#define CLV_PFD 1        // prefetch distance in trips
+#endif
+#ifndef CLV_PFZ
+#define CLV_PFZ 1        // L1 prefetch of the eta_s-neighbour planes one trip ahead (they are the loads that miss L1)
+#endif
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 #ifndef CLV_MINB
 #define CLV_MINB 2
 #endif
@@ -110,6 +169,7 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
   for (int m = 0; m < 14; ++m) S[m] = R(0);
   R cfl0 = R(0), cfl1 = R(0), cfl2 = R(0);
   const R tf = a.milne ? a.tau : R(1);
+  const R th2 = R(2) * a.theta;
 
   // ---- KT flux divergence, axes x, y, eta (Eq.40; A22) -------------------------------------------
   // fully unrolled: with ax a compile-time constant every field offset and the P delta^{a mu} select are
@@ -123,6 +183,14 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
 #pragma unroll
     for (int p = 0; p < 5; ++p) pp[p] = in + idx[p];
     const int o_ua = (1 + ax) * FS, o_ca = OX + (X_CX + ax) * FS;
+    if (CLV_PFZ && USE_PI && ax == 2) {      // first pi trip of this axis: in flight behind the T-field part
+#pragma unroll
+      for (int p = 0; p < 5; ++p)
+        if (p != 2) {
+#pragma unroll
+          for (int m = 0; m < 2 * CLV_PFD; ++m) prefetch_l1(pp[p] + (F_PI + m) * FS);
+        }
+    }
 
     R g[5], ua[5];
     R cl, cr;
@@ -145,6 +213,29 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
         const R w = pp[p][0] + Pp[p];
         wq[p] = w * g[p]; wa[p] = w * ua[p];
       }
+      if constexpr (CLV_PACK32 && sizeof(R) == 4) {
+        // packed pairs (mu = 0,1) and (2,3): Q, F and the whole flux difference as f32x2
+#pragma unroll
+        for (int hp = 0; hp < 2; ++hp) {
+          const int m0 = 2 * hp, m1 = m0 + 1;
+          const int o_t0 = (F_PI + m0) * FS, o_t1 = (F_PI + m1) * FS;
+          const int o_a0 = (F_PI + c_pidx[ax + 1][m0]) * FS, o_a1 = (F_PI + c_pidx[ax + 1][m1]) * FS;
+          F2 q[5], f[5];
+#pragma unroll
+          for (int p = 0; p < 5; ++p) {
+            const F2 um = {m0 == 0 ? (float)g[p] : (float)pp[p][m0 * FS], (float)pp[p][m1 * FS]};
+            F2 cq = {m0 == 0 ? -(float)Pp[p] : 0.0f, 0.0f};
+            F2 cf = {m0 == ax + 1 ? (float)Pp[p] : 0.0f, m1 == ax + 1 ? (float)Pp[p] : 0.0f};
+            if (USE_PI) {
+              cq.x += (float)pp[p][o_t0]; cq.y += (float)pp[p][o_t1];
+              cf.x += (float)pp[p][o_a0]; cf.y += (float)pp[p][o_a1];
+            }
+            q[p] = fma2(bc2((float)wq[p]), um, cq); f[p] = fma2(bc2((float)wa[p]), um, cf);
+          }
+          const F2 d = kt_div2_2(q, f, bc2((float)cl), bc2(-(float)cr), bc2((float)th2));
+          S[m0] -= R(d.x) * sc_T; S[m1] -= R(d.y) * sc_T;
+        }
+      } else {
 #pragma unroll
       for (int mu = 0; mu < 4; ++mu) {
         R q[5], f[5];
@@ -159,7 +250,8 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
           if (USE_PI) { tq += pp[p][o_t]; tfl += pp[p][o_a]; }
           q[p] = tq; f[p] = tfl;
         }
-        S[mu] -= kt_div2(q, f, cl, cr, a.theta) * sc_T;
+        S[mu] -= kt_div2(q, f, cl, cr, th2) * sc_T;
+      }
       }
     }
     // pi fields: Q = u^tau pi, F_a = u^a pi   (Eq.29)
@@ -170,9 +262,40 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
 #pragma unroll
       for (int p = 0; p < 5; ++p) pq[p] = pp[p] + F_PI * FS;
       R* slot = &sS[tid];
+      if constexpr (CLV_PACK32 && sizeof(R) == 4) {
+        F2 g2[5], ua2[5];
+#pragma unroll
+        for (int p = 0; p < 5; ++p) { g2[p] = bc2((float)g[p]); ua2[p] = bc2((float)ua[p]); }
+        const F2 cl2 = bc2((float)cl), ncr2 = bc2(-(float)cr), th22 = bc2((float)th2);
+#pragma unroll 1
+        for (int t = 0; t < 5; ++t) {
+          F2 q[5], f[5];
+          if (CLV_PFZ && ax == 2) {
+#pragma unroll
+            for (int p = 0; p < 5; ++p)
+              if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
+          }
+#pragma unroll
+          for (int p = 0; p < 5; ++p) {
+            const F2 v = {(float)pq[p][0], (float)pq[p][FS]};
+            q[p] = mul2(g2[p], v); f[p] = mul2(ua2[p], v);
+            pq[p] += 2 * FS;
+          }
+          const F2 d = kt_div2_2(q, f, cl2, ncr2, th22);
+          const R da = R(d.x) * sc_pi, db = R(d.y) * sc_pi;
+          slot[0] = (ax == 0) ? -da : slot[0] - da;
+          slot[256] = (ax == 0) ? -db : slot[256] - db;
+          slot += 2 * 256;
+        }
+      } else {
 #pragma unroll 1
       for (int t = 0; t < 5; ++t) {
         R qa[5], fa[5], qb[5], fb[5];
+        if (CLV_PFZ && ax == 2) {      // next trip's fields on the four off-centre planes
+#pragma unroll
+          for (int p = 0; p < 5; ++p)
+            if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
+        }
 #pragma unroll
         for (int p = 0; p < 5; ++p) {
           const R va = pq[p][0], vb = pq[p][FS];
@@ -180,11 +303,12 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
           qb[p] = g[p] * vb; fb[p] = ua[p] * vb;
           pq[p] += 2 * FS;
         }
-        const R da = kt_div2(qa, fa, cl, cr, a.theta) * sc_pi;
-        const R db = kt_div2(qb, fb, cl, cr, a.theta) * sc_pi;
+        const R da = kt_div2(qa, fa, cl, cr, th2) * sc_pi;
+        const R db = kt_div2(qb, fb, cl, cr, th2) * sc_pi;
         slot[0] = (ax == 0) ? -da : slot[0] - da;
         slot[256] = (ax == 0) ? -db : slot[256] - db;
         slot += 2 * 256;
+      }
       }
     }
   }

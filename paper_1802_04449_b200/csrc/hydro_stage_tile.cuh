@@ -147,9 +147,9 @@ __device__ __forceinline__ void qf(const R* __restrict__ pt, const PtAux<R>& x, 
 }
 // half-slope states of a cell: Q^l = Q + s/2 (left state of its upper face), Q^r = Q - s/2   (Eq.43-44, A4)
 template <typename R>
-__device__ __forceinline__ void lr(R Qm, R Q0, R Qp, R theta, R& L, R& Rr) {
-  const R s = hmm(Q0 - Qm, Qp - Q0, theta);
-  L = Q0 + s; Rr = Q0 - s;
+__device__ __forceinline__ void lr(R Qm, R Q0, R Qp, R th2, R& L, R& Rr) {
+  const R s4 = hmm4(Q0 - Qm, Qp - Q0, th2);      // 4 x the half slope
+  L = R(0.25) * s4 + Q0; Rr = R(-0.25) * s4 + Q0;
 }
 // 2 H_{i+1/2} from the left state of cell i and the right state of cell i+1   (Eq.41-42, A5)
 template <typename R>
@@ -332,6 +332,7 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
   PlaneAux<R> h1 = {R(1), R(0), R(0), R(0), R(0)}, h2 = h1;      // planes p-1 and p-2
   R km1[4] = {R(1), R(0), R(0), R(0)};                            // u~^mu of plane k-1
   const R tf = a.milne ? a.tau : R(1);
+  const R th2 = R(2) * a.theta;
   const R sc_eta = R(0.5) * a.scale[2], sc_x = R(0.5) * a.scale[0], sc_y = R(0.5) * a.scale[1];
   R cfl0 = R(0), cfl1 = R(0), cfl2 = R(0), emax = R(0);
 
@@ -389,8 +390,8 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
             qf<R, USE_PI, 0, false>(pt - 1, xm, f, Qm, Fm); qf<R, USE_PI, 0, false>(pt, xin, f, Q0, F0);
             qf<R, USE_PI, 0, false>(pt + 1, xpl, f, Qp, Fp);
           }
-          lr(Qm, Q0, Qp, a.theta, QL, QR);
-          lr(Fm, F0, Fp, a.theta, FL, FR);
+          lr(Qm, Q0, Qp, th2, QL, QR);
+          lr(Fm, F0, Fp, th2, FL, FR);
           sm.xh[t & 1][slot][side][0][r] = side ? QR : QL;
           sm.xh[t & 1][slot][side][1][r] = side ? FR : FL;
         } else if (row >= 2 && row <= 5) {     // y: warp = (side, field of the trip), lanes along x
@@ -408,8 +409,8 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
             qf<R, USE_PI, 1, false>(pt - SX, ya, f, Qm, Fm); qf<R, USE_PI, 1, false>(pt, yb, f, Q0, F0);
             qf<R, USE_PI, 1, false>(pt + SX, yc, f, Qp, Fp);
           }
-          lr(Qm, Q0, Qp, a.theta, QL, QR);
-          lr(Fm, F0, Fp, a.theta, FL, FR);
+          lr(Qm, Q0, Qp, th2, QL, QR);
+          lr(Fm, F0, Fp, th2, FL, FR);
           sm.yh[t % 3][slot][side][0][lane] = side ? QR : QL;
           sm.yh[t % 3][slot][side][1][lane] = side ? FR : FL;
         }
@@ -486,8 +487,8 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
           qf<R, USE_PI, 2, IS_T>(rp, zp, f, Qp, Fp);
           qf<R, USE_PI, 2, IS_T>(r1, z1, f, Q1, F1);
           qf<R, USE_PI, 2, IS_T>(rk, z2, f, Q2, F2);
-          lr(Q2, Q1, Qp, a.theta, QL1, QR1);
-          lr(F2, F1, Fp, a.theta, FL1, FR1);
+          lr(Q2, Q1, Qp, th2, QL1, QR1);
+          lr(F2, F1, Fp, th2, FL1, FR1);
           const R Hn = face2(QLk, FLk, QR1, FR1, cface);
           Sf = -(Hn - Hk) * (sc_eta * tfac);
           priv.put_kept(f, QL1, FL1, Hn);
@@ -498,8 +499,8 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
             qf<R, USE_PI, 0, IS_T>(rk - 1, xm, f, Qm, Fm);
             qf<R, USE_PI, 0, IS_T>(rk, x0, f, Q0, F0);
             qf<R, USE_PI, 0, IS_T>(rk + 1, xpl, f, Qp, Fp);
-            lr(Qm, Q0, Qp, a.theta, QL, QR);
-            lr(Fm, F0, Fp, a.theta, FL, FR);
+            lr(Qm, Q0, Qp, th2, QL, QR);
+            lr(Fm, F0, Fp, th2, FL, FR);
             R QRn = shfl_dn_(QR), FRn = shfl_dn_(FR);
             if (lane == TX - 1) { QRn = sm.xh[t & 1][slot][1][0][row]; FRn = sm.xh[t & 1][slot][1][1][row]; }
             const R Hr = face2(QL, FL, QRn, FRn, cr);
@@ -512,8 +513,8 @@ stage_tile_kernel(const TileArgs<R> a, const __grid_constant__ CUtensorMap tmap)
             qf<R, USE_PI, 1, IS_T>(rk - SX, ym, f, Qm, Fm);
             qf<R, USE_PI, 1, IS_T>(rk, y0, f, Q0, F0);
             qf<R, USE_PI, 1, IS_T>(rk + SX, ypl, f, Qp, Fp);
-            lr(Qm, Q0, Qp, a.theta, QLy, QRy);
-            lr(Fm, F0, Fp, a.theta, FLy, FRy);
+            lr(Qm, Q0, Qp, th2, QLy, QRy);
+            lr(Fm, F0, Fp, th2, FLy, FRy);
             sm.yx[t & 1][slot][0][row][lane] = QLy; sm.yx[t & 1][slot][1][row][lane] = FLy;
             sm.yx[t & 1][slot][2][row][lane] = QRy; sm.yx[t & 1][slot][3][row][lane] = FRy;
           }

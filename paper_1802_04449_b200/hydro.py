@@ -226,7 +226,7 @@ class Hydro:
         return int(self._lib.hydro_launch_count(self._h))
 
     def kernel(self) -> int:
-        """The stage kernel in use (1 reference, 2 per-cell fused, 3 tile); kernel=0 resolves by precision."""
+        """The stage kernel in use (1 reference, 2 per-cell fused, 3 tile); kernel=0 resolves to the fastest measured (2)."""
         return int(self._lib.hydro_kernel(self._h))
 
     def close(self):
