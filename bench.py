@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused viscous KT-RK2 step (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--precision 64|32] [--kernel 0|1|2|3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--precision 64|32] [--kernel 0|1|2|3|4]
     python bench.py --impl reference ...      # the CPU oracle, timed as it stands (bounded sample per step)
 
 A "step" is one full RK2 step (both stages: KT fluxes of T^{tau mu} and pi^{mu nu} on three axes, Milne and
@@ -166,7 +166,7 @@ def roofline_record(cells, precision, viscous, ms_total, launches, kernel, count
     c = counters.get(f"f{precision}_k{kernel}", {}) if viscous else {}
     rec = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
            "traffic": c.get("dram_bytes_per_launch"), "peak_source": peak_src,
-           "kernel": {1: "stage_ref_kernel", 2: "stage_fused_kernel", 3: "stage_tile_kernel"}[kernel] +
+           "kernel": {1: "stage_ref_kernel", 2: "stage_fused_kernel", 3: "stage_tile_kernel", 4: "stage_march_kernel"}[kernel] +
                      " (average of the stage-1 and stage-2 launches)",
            "algorithmic_bytes_per_launch": algo_per_launch, "avg_launch_ms": avg_launch_s * 1e3}
     # second view: what actually limits the kernel is instruction issue / fp64 latency, not HBM.

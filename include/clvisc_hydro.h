@@ -72,10 +72,12 @@ typedef struct {
  * <= 0 selects the default 0.999 (gamma <= 22.4; A7 gives the evidence); root_iters: fixed Newton iteration
  * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
  * stream); workspace: DEVICE memory of at least hydro_workspace_bytes(), 256-byte aligned.
- * kernel: 0 = default (the faster one as measured on B200: 2 in both precisions);
+ * kernel: 0 = default (the fastest one as measured on B200: 4 in both precisions);
+ * 4 = marching per-cell kernel (hydro_stage_march.cuh): kernel 2's store and x / y flux code, but a block walks along
+ * eta_s and forms every eta_s slope and face once, with the per-column pipeline state in tensor memory;
  * 2 = per-cell fused kernel on the extended 19-word state (hydro_stage_fused.cuh); 3 = tile kernel
  * (hydro_stage_tile.cuh): TMA-staged 32x8 tiles marching along eta_s, every slope and face flux computed once, 14-word
- * ghosted SoA state; 1 = per-cell reference kernel (re-derives P, u^tau, c_a at every stencil point).  All three give
+ * ghosted SoA state; 1 = per-cell reference kernel (re-derives P, u^tau, c_a at every stencil point).  All four give
  * the same results to rounding and are covered by the parity tests. */
 typedef struct {
   int precision;
@@ -128,13 +130,42 @@ int hydro_step(hydro_ctx *ctx, int n);
  * NULL.  Synchronises the stream when mem == HYDRO_MEM_HOST. */
 int hydro_read(hydro_ctx *ctx, void *e, void *u, void *pi, int mem);
 
+/* ---- Freeze-out hypersurface ------------------------------------------------------------------
+ * PAPER.md:268 (text under Eq.55): d Sigma_mu is the surface element of the hypersurface of constant freeze-out energy
+ * density e_frz; it is found on the GPU during the evolution, next to the e_max reduction that stops the
+ * run, so the full field never leaves the device.  The paper does not print the finder; reading A27: the
+ * cuboidal surface between two stored time levels a and b (faces between hot, e >= e_frz, and cold 4-D cells; crossing
+ * point and fluid state by linear interpolation in e).
+ *
+ * hydro_freezeout_bytes: size of the DEVICE workspace (two stored levels of 15 words per cell + counters).
+ * hydro_freezeout_begin: stores the current state as level a, resets the element counter and the slab index.  The
+ *   workspace is caller-owned, 256-byte aligned, and must stay alive while the finder is in use.
+ * hydro_freezeout_slab: takes the current state as level b, APPENDS the elements between a and b to keys / rows
+ *   (DEVICE arrays of `capacity` int64 keys and capacity x 22 doubles; unordered), then b becomes the new a.
+ *     key  = (slab * 4 + dir) * N + cell      dir 0: time-like face of the cell; 1,2,3: face towards +x, +y, +eta_s
+ *                                             cell = (k * ny + j) * nx + i; N = nx ny nz
+ *     row  = [0:4] tau, x, y, eta_s of the crossing point   [4:8] d Sigma~_mu (covariant tilde components, normal
+ *            pointing to the cold side)   [8:11] u~^i   [11] u~^tau   [12:22] pi~ (order of the header)
+ *   fp64 arithmetic in both precisions.  *n_total = elements since begin (also those that did not fit), *n_hot = hot
+ *   cells of level b (0 <=> e_max < e_frz, the paper's stop criterion).  Synchronises the stream (16 bytes come back).
+ *   Returns HYDRO_ENOMEM when n_total exceeds capacity (the elements that did not fit are dropped), HYDRO_ESTATE before
+ *   hydro_freezeout_begin.
+ * hydro_freezeout_run: repeats { hydro_step(steps_per_slab); hydro_freezeout_slab } until no hot cell is left or
+ *   max_slabs slabs are done; *n_slabs = slabs done. */
+size_t hydro_freezeout_bytes(const hydro_grid *grid, int precision);
+int hydro_freezeout_begin(hydro_ctx *ctx, void *workspace, size_t workspace_bytes, double e_frz);
+int hydro_freezeout_slab(hydro_ctx *ctx, long long *keys, double *rows, long long capacity,
+                         long long *n_total, long long *n_hot);
+int hydro_freezeout_run(hydro_ctx *ctx, int steps_per_slab, int max_slabs, long long *keys, double *rows,
+                        long long capacity, long long *n_total, int *n_slabs);
+
 /* Copy the diagnostics to the host (synchronises the stream).  Returns a warning mask. */
 int hydro_diag(hydro_ctx *ctx, hydro_diag_t *out);
 
 /* Number of kernel launches issued by this context since create (host counter). */
 long long hydro_launch_count(const hydro_ctx *ctx);
 
-/* The stage kernel this context runs (1, 2 or 3): opts->kernel, or what 0 resolved to. */
+/* The stage kernel this context runs (1, 2, 3 or 4): opts->kernel, or what 0 resolved to. */
 int hydro_kernel(const hydro_ctx *ctx);
 
 void hydro_destroy(hydro_ctx *ctx);

@@ -27,6 +27,8 @@
 #include "hydro_stage_ref.cuh"
 #include "hydro_stage_fused.cuh"
 #include "hydro_stage_tile.cuh"
+#include "hydro_stage_march.cuh"
+#include "hydro_freezeout.cuh"
 
 namespace clv {
 
@@ -46,10 +48,10 @@ struct Layout {
   size_t off_diag, off_eos, off_buf[3], off_gstar, total;
 };
 
-// kernel 0 = the faster one as measured on B200 at 301x301x201 (round 2): the per-cell fused
-// kernel in both precisions (fp64 14.4 vs 15.7 ms per step; fp32 7.6 vs 8.0 once the FMNMX minmod and the packed f32x2
-// arithmetic are in: the tile kernel cannot hide its latencies with 8 (fp64) / 16 (fp32) warps per SM)
-static int resolve_kernel(int kernel, int precision) { (void)precision; return kernel != 0 ? kernel : 2; }
+// kernel 0 = the fastest one as measured on B200 at 301x301x201 (round 2): the marching per-cell
+// kernel (4) in both precisions: fp64 13.4 ms per step against 14.4 (kernel 2) and 15.7 (kernel 3); fp32 6.95 against
+// 7.5 and 8.0.
+static int resolve_kernel(int kernel, int precision) { (void)precision; return kernel != 0 ? kernel : 4; }
 
 static bool make_layout(const hydro_grid* g, int precision, double eta_s, int kernel, Layout* L) {
   if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;
@@ -292,6 +294,14 @@ struct hydro_ctx {
   // kernel 3: TMA tensor maps of the three state buffers with box depth nf ([b][0]) and 4 ([b][1]); tiling
   CUtensorMap tmap[3][2];
   int ntx, nty, nchunk, chunk;
+  int march_chunk;   // kernel 4: eta_s planes per block
+  // freeze-out surface finder: caller-owned workspace [counters 256 B][level 0][level 1], each level
+  // = e, u~^mu[4], pi~[10] in the user layout; level[frz_a] is the stored level a
+  char* frz_ws;
+  void* frz_level[2];
+  int frz_a;
+  double frz_e, frz_tau_a;
+  long long frz_slab;
 };
 
 namespace {
@@ -461,7 +471,9 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
 
 template <typename R, bool VISC, int MODE>
 int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
-  if (c->kernel == 2) {
+  if (c->kernel == 4 && MODE != 0) {
+    if constexpr (MODE != 0) launch_stage_march<R, VISC, MODE>(a, c->march_chunk, c->stream);
+  } else if (c->kernel == 2 || c->kernel == 4) {      // the bootstrap of kernel 4 runs in the per-cell kernel (same store)
     launch_stage_fused<R, VISC, MODE>(a, c->stream);
   } else {
     dim3 block(32, 8, 1);
@@ -646,6 +658,18 @@ int do_history(hydro_ctx* c, void* user, int mem, int dir) {
   return HYDRO_OK;
 }
 
+// freeze-out finder: bytes of one stored level; store the current state as level `which`
+static size_t frz_level_bytes(const hydro_grid* g, int precision) {
+  const size_t N = (size_t)g->nx * g->ny * g->nz;
+  return align_up((size_t)15 * N * (precision == 64 ? 8 : 4), 256);
+}
+template <typename R>
+int frz_store_level(hydro_ctx* c, int which) {
+  const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
+  R* lv = static_cast<R*>(c->frz_level[which]);
+  return do_read<R>(c, lv, lv + N, lv + 5 * N, HYDRO_MEM_DEVICE);
+}
+
 }  // namespace
 
 extern "C" {
@@ -663,7 +687,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   *out = nullptr;
   if (!grid || !eos || !opts) return HYDRO_EINVAL;
   Layout L;
-  if (opts->kernel < 0 || opts->kernel > 3) return HYDRO_EINVAL;
+  if (opts->kernel < 0 || opts->kernel > 4) return HYDRO_EINVAL;
   if (!make_layout(grid, opts->precision, eta_over_s, opts->kernel, &L)) return HYDRO_EINVAL;
   if (!(dtau > 0.0) || !(grid->dx > 0.0) || !(grid->dy > 0.0) || !(grid->deta > 0.0)) return HYDRO_EINVAL;
   if (grid->geometry != 0 && grid->geometry != 1) return HYDRO_EINVAL;
@@ -705,6 +729,13 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->cur = 0; c->prev = 1; c->step = 0; c->launches = 0; c->loaded = false;
   int rc = opts->precision == 64 ? upload_eos<double>(c, eos, &c->eos64) : upload_eos<float>(c, eos, &c->eos32);
   if (rc == HYDRO_OK && cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) rc = HYDRO_ECUDA;
+  if (rc == HYDRO_OK && c->kernel == 4) {
+    if (L.sz >= (1ll << 31)) rc = HYDRO_EINVAL;      // kernel 4 keeps in-plane offsets in 32 bits
+    int dev = 0, nsm = 148;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+      rc = HYDRO_ECUDA;
+    c->march_chunk = march_chunk(grid->nx, grid->ny, grid->nz, nsm > 0 ? nsm : 148);
+  }
   if (rc == HYDRO_OK && L.soa) {
     int dev = 0, nsm = 148;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
@@ -755,6 +786,84 @@ int hydro_read(hydro_ctx* c, void* e, void* u, void* pi, int mem) {
   if (!c || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
   if (!c->loaded) return HYDRO_ESTATE;
   return c->precision == 64 ? do_read<double>(c, e, u, pi, mem) : do_read<float>(c, e, u, pi, mem);
+}
+
+
+// ---- freeze-out hypersurface (hydro_freezeout.cuh) ----------------------------------------------------
+
+size_t hydro_freezeout_bytes(const hydro_grid* grid, int precision) {
+  if (!grid || grid->nx < 1 || grid->ny < 1 || grid->nz < 1 || (precision != 64 && precision != 32)) return 0;
+  return 256 + 2 * frz_level_bytes(grid, precision);
+}
+
+int hydro_freezeout_begin(hydro_ctx* c, void* workspace, size_t bytes, double e_frz) {
+  if (!c || !workspace || !(e_frz > 0.0)) return HYDRO_EINVAL;
+  if (!c->loaded) return HYDRO_ESTATE;
+  if (bytes < hydro_freezeout_bytes(&c->grid, c->precision) || (reinterpret_cast<size_t>(workspace) & 255))
+    return HYDRO_ENOMEM;
+  c->frz_ws = static_cast<char*>(workspace);
+  c->frz_level[0] = c->frz_ws + 256;
+  c->frz_level[1] = c->frz_ws + 256 + frz_level_bytes(&c->grid, c->precision);
+  c->frz_a = 0; c->frz_e = e_frz; c->frz_slab = 0;
+  c->frz_tau_a = c->tau0 + (double)c->step * c->dtau;
+  if (cudaMemsetAsync(c->frz_ws, 0, 256, c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  return c->precision == 64 ? frz_store_level<double>(c, 0) : frz_store_level<float>(c, 0);
+}
+
+int hydro_freezeout_slab(hydro_ctx* c, long long* keys, double* rows, long long capacity, long long* n_total,
+                         long long* n_hot) {
+  if (!c || capacity < 0 || (capacity > 0 && (!keys || !rows))) return HYDRO_EINVAL;
+  if (!c->loaded || !c->frz_ws) return HYDRO_ESTATE;
+  const int b = c->frz_a ^ 1;
+  int rc = c->precision == 64 ? frz_store_level<double>(c, b) : frz_store_level<float>(c, b);
+  if (rc) return rc;
+  FrzArgs a;
+  memset(&a, 0, sizeof(a));
+  a.nx = c->grid.nx; a.ny = c->grid.ny; a.nz = c->grid.nz;
+  for (int d = 0; d < 3; ++d) a.bc[d] = c->grid.bc[d];
+  a.milne = c->grid.geometry == 0 ? 1 : 0;
+  a.N = (long long)a.nx * a.ny * a.nz;
+  a.dx = c->grid.dx; a.dy = c->grid.dy; a.de = c->grid.deta;
+  a.tau_a = c->frz_tau_a; a.tau_b = c->tau0 + (double)c->step * c->dtau; a.e_frz = c->frz_e;
+  a.slab = c->frz_slab; a.capacity = capacity;
+  a.cnt = reinterpret_cast<FrzCounters*>(c->frz_ws);
+  a.keys = keys; a.rows = rows;
+  if (cudaMemsetAsync(&a.cnt->n_hot_b, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  const unsigned nb = (unsigned)((a.N + 255) / 256);
+  if (c->precision == 64) {
+    const double* la = static_cast<const double*>(c->frz_level[c->frz_a]);
+    const double* lb = static_cast<const double*>(c->frz_level[b]);
+    freezeout_kernel<double><<<nb, 256, 0, c->stream>>>(a, la, la + a.N, la + 5 * a.N, lb, lb + a.N, lb + 5 * a.N);
+  } else {
+    const float* la = static_cast<const float*>(c->frz_level[c->frz_a]);
+    const float* lb = static_cast<const float*>(c->frz_level[b]);
+    freezeout_kernel<float><<<nb, 256, 0, c->stream>>>(a, la, la + a.N, la + 5 * a.N, lb, lb + a.N, lb + 5 * a.N);
+  }
+  c->launches += 1;
+  if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
+  FrzCounters h;
+  if (cudaMemcpyAsync(&h, a.cnt, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  c->frz_a = b; c->frz_tau_a = a.tau_b; c->frz_slab += 1;
+  if (n_total) *n_total = (long long)h.n_elem;
+  if (n_hot) *n_hot = (long long)h.n_hot_b;
+  return (long long)h.n_elem > capacity ? HYDRO_ENOMEM : HYDRO_OK;
+}
+
+int hydro_freezeout_run(hydro_ctx* c, int steps_per_slab, int max_slabs, long long* keys, double* rows,
+                        long long capacity, long long* n_total, int* n_slabs) {
+  if (!c || steps_per_slab < 1 || max_slabs < 0) return HYDRO_EINVAL;
+  if (!c->loaded || !c->frz_ws) return HYDRO_ESTATE;
+  int done = 0, rc = HYDRO_OK;
+  long long hot = 1;
+  while (done < max_slabs && hot > 0) {
+    if ((rc = hydro_step(c, steps_per_slab))) break;
+    rc = hydro_freezeout_slab(c, keys, rows, capacity, n_total, &hot);
+    if (rc) break;
+    done += 1;
+  }
+  if (n_slabs) *n_slabs = done;
+  return rc;
 }
 
 int hydro_diag(hydro_ctx* c, hydro_diag_t* out) {

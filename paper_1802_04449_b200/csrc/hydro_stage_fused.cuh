@@ -144,6 +144,143 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 #define CLV_MINB32 2     // fp32 blocks per SM; with the unrolled axis loop 2 (128 registers, no spills) measured 9.25 ms
                          // per step against 9.9 (3 blocks, 80 registers) and 9.5 (4 blocks, 64 registers)
 #endif
+// KT flux difference (Eq.40-44) of every evolved field along axis AX from the five-point star pp[0..4] of the extended
+// state (pp[2] = the cell itself).  T fields: S[0..3] -= ...; pi fields: the thread-private shared-memory slots
+// slot0[m * 256] (INIT: first axis, "=" instead of "-=").  cfl = c_a h / Delta_a of the cell.  Shared by the per-cell
+// kernel (three axes) and the marching kernel (x and y; hydro_stage_march.cuh).
+template <typename R, bool USE_PI, int AX, bool INIT, int OX, typename A>
+__device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ const (&pp)[5], R th2, R tf, R (&S)[14],
+                                          R* slot0, R& cfl) {
+  const int o_ua = (1 + AX) * FS, o_ca = OX + (X_CX + AX) * FS;
+  if (CLV_PFZ && USE_PI && AX == 2) {      // first pi trip of this axis: in flight behind the T-field part
+#pragma unroll
+    for (int p = 0; p < 5; ++p)
+      if (p != 2) {
+#pragma unroll
+        for (int m = 0; m < 2 * CLV_PFD; ++m) prefetch_l1(pp[p] + (F_PI + m) * FS);
+      }
+  }
+
+  R g[5], ua[5];
+  R cl, cr;
+  {
+    const R c1 = pp[1][o_ca], c2 = pp[2][o_ca], c3 = pp[3][o_ca];
+    cl = max_(c1, c2); cr = max_(c2, c3);
+    cfl = c2 * a.h * a.scale[AX];
+  }
+#pragma unroll
+  for (int p = 0; p < 5; ++p) { g[p] = pp[p][OX + X_G * FS]; ua[p] = pp[p][o_ua]; }
+  const R sc_pi = R(0.5) * a.scale[AX], sc_T = sc_pi * tf;
+
+  {
+    // T fields: Q^mu/tau = T_f^{tau mu}, F_a^mu/tau = T_f^{a mu}   (Eq.27, Eq.39)
+    R wq[5], wa[5], Pp[5];
+#pragma unroll
+    for (int p = 0; p < 5; ++p) {
+      Pp[p] = pp[p][OX + X_P * FS];
+      const R w = pp[p][0] + Pp[p];
+      wq[p] = w * g[p]; wa[p] = w * ua[p];
+    }
+    if constexpr (CLV_PACK32 && sizeof(R) == 4) {
+      // packed pairs (mu = 0,1) and (2,3): Q, F and the whole flux difference as f32x2
+#pragma unroll
+      for (int hp = 0; hp < 2; ++hp) {
+        const int m0 = 2 * hp, m1 = m0 + 1;
+        const int o_t0 = (F_PI + m0) * FS, o_t1 = (F_PI + m1) * FS;
+        const int o_a0 = (F_PI + c_pidx[AX + 1][m0]) * FS, o_a1 = (F_PI + c_pidx[AX + 1][m1]) * FS;
+        F2 q[5], f[5];
+#pragma unroll
+        for (int p = 0; p < 5; ++p) {
+          const F2 um = {m0 == 0 ? (float)g[p] : (float)pp[p][m0 * FS], (float)pp[p][m1 * FS]};
+          F2 cq = {m0 == 0 ? -(float)Pp[p] : 0.0f, 0.0f};
+          F2 cf = {m0 == AX + 1 ? (float)Pp[p] : 0.0f, m1 == AX + 1 ? (float)Pp[p] : 0.0f};
+          if (USE_PI) {
+            cq.x += (float)pp[p][o_t0]; cq.y += (float)pp[p][o_t1];
+            cf.x += (float)pp[p][o_a0]; cf.y += (float)pp[p][o_a1];
+          }
+          q[p] = fma2(bc2((float)wq[p]), um, cq); f[p] = fma2(bc2((float)wa[p]), um, cf);
+        }
+        const F2 d = kt_div2_2(q, f, bc2((float)cl), bc2(-(float)cr), bc2((float)th2));
+        S[m0] -= R(d.x) * sc_T; S[m1] -= R(d.y) * sc_T;
+      }
+    } else {
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+      R q[5], f[5];
+      const int o_t = (F_PI + (mu == 0 ? 0 : mu)) * FS;            // pi^{tau mu}: components 0..3
+      const int o_a = (F_PI + c_pidx[AX + 1][mu]) * FS;            // pi^{a mu} (a constant-memory lookup measured
+                                                                   // faster than a constexpr index here)
+#pragma unroll
+      for (int p = 0; p < 5; ++p) {
+        const R umu = mu == 0 ? g[p] : pp[p][mu * FS];
+        R tq = wq[p] * umu - (mu == 0 ? Pp[p] : R(0));
+        R tfl = wa[p] * umu + (mu == AX + 1 ? Pp[p] : R(0));
+        if (USE_PI) { tq += pp[p][o_t]; tfl += pp[p][o_a]; }
+        q[p] = tq; f[p] = tfl;
+      }
+      S[mu] -= kt_div2(q, f, cl, cr, th2) * sc_T;
+    }
+    }
+  }
+  // pi fields: Q = u^tau pi, F_a = u^a pi   (Eq.29)
+  if (USE_PI) {
+    // two fields per trip: their 12 minmod chains interleave (ILP for the 4 warps per scheduler), the field
+    // offsets inside a trip are immediates and the five star pointers are bumped once per trip
+    const R* __restrict__ pq[5];
+#pragma unroll
+    for (int p = 0; p < 5; ++p) pq[p] = pp[p] + F_PI * FS;
+    R* slot = slot0;
+    if constexpr (CLV_PACK32 && sizeof(R) == 4) {
+      F2 g2[5], ua2[5];
+#pragma unroll
+      for (int p = 0; p < 5; ++p) { g2[p] = bc2((float)g[p]); ua2[p] = bc2((float)ua[p]); }
+      const F2 cl2 = bc2((float)cl), ncr2 = bc2(-(float)cr), th22 = bc2((float)th2);
+#pragma unroll 1
+      for (int t = 0; t < 5; ++t) {
+        F2 q[5], f[5];
+        if (CLV_PFZ && AX == 2) {
+#pragma unroll
+          for (int p = 0; p < 5; ++p)
+            if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
+        }
+#pragma unroll
+        for (int p = 0; p < 5; ++p) {
+          const F2 v = {(float)pq[p][0], (float)pq[p][FS]};
+          q[p] = mul2(g2[p], v); f[p] = mul2(ua2[p], v);
+          pq[p] += 2 * FS;
+        }
+        const F2 d = kt_div2_2(q, f, cl2, ncr2, th22);
+        const R da = R(d.x) * sc_pi, db = R(d.y) * sc_pi;
+        slot[0] = INIT ? -da : slot[0] - da;
+        slot[256] = INIT ? -db : slot[256] - db;
+        slot += 2 * 256;
+      }
+    } else {
+#pragma unroll 1
+    for (int t = 0; t < 5; ++t) {
+      R qa[5], fa[5], qb[5], fb[5];
+      if (CLV_PFZ && AX == 2) {      // next trip's fields on the four off-centre planes
+#pragma unroll
+        for (int p = 0; p < 5; ++p)
+          if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
+      }
+#pragma unroll
+      for (int p = 0; p < 5; ++p) {
+        const R va = pq[p][0], vb = pq[p][FS];
+        qa[p] = g[p] * va; fa[p] = ua[p] * va;
+        qb[p] = g[p] * vb; fb[p] = ua[p] * vb;
+        pq[p] += 2 * FS;
+      }
+      const R da = kt_div2(qa, fa, cl, cr, th2) * sc_pi;
+      const R db = kt_div2(qb, fb, cl, cr, th2) * sc_pi;
+      slot[0] = INIT ? -da : slot[0] - da;
+      slot[256] = INIT ? -db : slot[256] - db;
+      slot += 2 * 256;
+    }
+    }
+  }
+}
+
 template <typename R, bool VISC, int MODE>
 __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB)) stage_fused_kernel(const StageArgs<R> a) {
   constexpr bool USE_PI = VISC && (MODE != 0);
@@ -182,135 +319,9 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
     const R* __restrict__ pp[5];
 #pragma unroll
     for (int p = 0; p < 5; ++p) pp[p] = in + idx[p];
-    const int o_ua = (1 + ax) * FS, o_ca = OX + (X_CX + ax) * FS;
-    if (CLV_PFZ && USE_PI && ax == 2) {      // first pi trip of this axis: in flight behind the T-field part
-#pragma unroll
-      for (int p = 0; p < 5; ++p)
-        if (p != 2) {
-#pragma unroll
-          for (int m = 0; m < 2 * CLV_PFD; ++m) prefetch_l1(pp[p] + (F_PI + m) * FS);
-        }
-    }
-
-    R g[5], ua[5];
-    R cl, cr;
-    {
-      const R c1 = pp[1][o_ca], c2 = pp[2][o_ca], c3 = pp[3][o_ca];
-      cl = max_(c1, c2); cr = max_(c2, c3);
-      const R cv = c2 * a.h * a.scale[ax];
-      if (ax == 0) cfl0 = cv; else if (ax == 1) cfl1 = cv; else cfl2 = cv;
-    }
-#pragma unroll
-    for (int p = 0; p < 5; ++p) { g[p] = pp[p][OX + X_G * FS]; ua[p] = pp[p][o_ua]; }
-    const R sc_pi = R(0.5) * a.scale[ax], sc_T = sc_pi * tf;
-
-    {
-      // T fields: Q^mu/tau = T_f^{tau mu}, F_a^mu/tau = T_f^{a mu}   (Eq.27, Eq.39)
-      R wq[5], wa[5], Pp[5];
-#pragma unroll
-      for (int p = 0; p < 5; ++p) {
-        Pp[p] = pp[p][OX + X_P * FS];
-        const R w = pp[p][0] + Pp[p];
-        wq[p] = w * g[p]; wa[p] = w * ua[p];
-      }
-      if constexpr (CLV_PACK32 && sizeof(R) == 4) {
-        // packed pairs (mu = 0,1) and (2,3): Q, F and the whole flux difference as f32x2
-#pragma unroll
-        for (int hp = 0; hp < 2; ++hp) {
-          const int m0 = 2 * hp, m1 = m0 + 1;
-          const int o_t0 = (F_PI + m0) * FS, o_t1 = (F_PI + m1) * FS;
-          const int o_a0 = (F_PI + c_pidx[ax + 1][m0]) * FS, o_a1 = (F_PI + c_pidx[ax + 1][m1]) * FS;
-          F2 q[5], f[5];
-#pragma unroll
-          for (int p = 0; p < 5; ++p) {
-            const F2 um = {m0 == 0 ? (float)g[p] : (float)pp[p][m0 * FS], (float)pp[p][m1 * FS]};
-            F2 cq = {m0 == 0 ? -(float)Pp[p] : 0.0f, 0.0f};
-            F2 cf = {m0 == ax + 1 ? (float)Pp[p] : 0.0f, m1 == ax + 1 ? (float)Pp[p] : 0.0f};
-            if (USE_PI) {
-              cq.x += (float)pp[p][o_t0]; cq.y += (float)pp[p][o_t1];
-              cf.x += (float)pp[p][o_a0]; cf.y += (float)pp[p][o_a1];
-            }
-            q[p] = fma2(bc2((float)wq[p]), um, cq); f[p] = fma2(bc2((float)wa[p]), um, cf);
-          }
-          const F2 d = kt_div2_2(q, f, bc2((float)cl), bc2(-(float)cr), bc2((float)th2));
-          S[m0] -= R(d.x) * sc_T; S[m1] -= R(d.y) * sc_T;
-        }
-      } else {
-#pragma unroll
-      for (int mu = 0; mu < 4; ++mu) {
-        R q[5], f[5];
-        const int o_t = (F_PI + (mu == 0 ? 0 : mu)) * FS;            // pi^{tau mu}: components 0..3
-        const int o_a = (F_PI + c_pidx[ax + 1][mu]) * FS;            // pi^{a mu} (a constant-memory lookup measured
-                                                                     // faster than a constexpr index here)
-#pragma unroll
-        for (int p = 0; p < 5; ++p) {
-          const R umu = mu == 0 ? g[p] : pp[p][mu * FS];
-          R tq = wq[p] * umu - (mu == 0 ? Pp[p] : R(0));
-          R tfl = wa[p] * umu + (mu == ax + 1 ? Pp[p] : R(0));
-          if (USE_PI) { tq += pp[p][o_t]; tfl += pp[p][o_a]; }
-          q[p] = tq; f[p] = tfl;
-        }
-        S[mu] -= kt_div2(q, f, cl, cr, th2) * sc_T;
-      }
-      }
-    }
-    // pi fields: Q = u^tau pi, F_a = u^a pi   (Eq.29)
-    if (USE_PI) {
-      // two fields per trip: their 12 minmod chains interleave (ILP for the 4 warps per scheduler), the field
-      // offsets inside a trip are immediates and the five star pointers are bumped once per trip
-      const R* __restrict__ pq[5];
-#pragma unroll
-      for (int p = 0; p < 5; ++p) pq[p] = pp[p] + F_PI * FS;
-      R* slot = &sS[tid];
-      if constexpr (CLV_PACK32 && sizeof(R) == 4) {
-        F2 g2[5], ua2[5];
-#pragma unroll
-        for (int p = 0; p < 5; ++p) { g2[p] = bc2((float)g[p]); ua2[p] = bc2((float)ua[p]); }
-        const F2 cl2 = bc2((float)cl), ncr2 = bc2(-(float)cr), th22 = bc2((float)th2);
-#pragma unroll 1
-        for (int t = 0; t < 5; ++t) {
-          F2 q[5], f[5];
-          if (CLV_PFZ && ax == 2) {
-#pragma unroll
-            for (int p = 0; p < 5; ++p)
-              if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
-          }
-#pragma unroll
-          for (int p = 0; p < 5; ++p) {
-            const F2 v = {(float)pq[p][0], (float)pq[p][FS]};
-            q[p] = mul2(g2[p], v); f[p] = mul2(ua2[p], v);
-            pq[p] += 2 * FS;
-          }
-          const F2 d = kt_div2_2(q, f, cl2, ncr2, th22);
-          const R da = R(d.x) * sc_pi, db = R(d.y) * sc_pi;
-          slot[0] = (ax == 0) ? -da : slot[0] - da;
-          slot[256] = (ax == 0) ? -db : slot[256] - db;
-          slot += 2 * 256;
-        }
-      } else {
-#pragma unroll 1
-      for (int t = 0; t < 5; ++t) {
-        R qa[5], fa[5], qb[5], fb[5];
-        if (CLV_PFZ && ax == 2) {      // next trip's fields on the four off-centre planes
-#pragma unroll
-          for (int p = 0; p < 5; ++p)
-            if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
-        }
-#pragma unroll
-        for (int p = 0; p < 5; ++p) {
-          const R va = pq[p][0], vb = pq[p][FS];
-          qa[p] = g[p] * va; fa[p] = ua[p] * va;
-          qb[p] = g[p] * vb; fb[p] = ua[p] * vb;
-          pq[p] += 2 * FS;
-        }
-        const R da = kt_div2(qa, fa, cl, cr, th2) * sc_pi;
-        const R db = kt_div2(qb, fb, cl, cr, th2) * sc_pi;
-        slot[0] = (ax == 0) ? -da : slot[0] - da;
-        slot[256] = (ax == 0) ? -db : slot[256] - db;
-        slot += 2 * 256;
-      }
-      }
-    }
+    if (ax == 0) axis_flux<R, USE_PI, 0, true, OX>(a, pp, th2, tf, S, &sS[tid], cfl0);
+    else if (ax == 1) axis_flux<R, USE_PI, 1, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl1);
+    else axis_flux<R, USE_PI, 2, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl2);
   }
   if (USE_PI) {
 #pragma unroll

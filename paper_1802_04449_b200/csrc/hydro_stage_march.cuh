@@ -1,0 +1,325 @@
+// hydro_stage_march.cuh -- "kernel 4": the per-cell fused stage kernel MARCHING along eta_s.
+//
+// Same field store (blocked extended state, 19 words per cell), same x / y flux code (axis_flux) and same stage tail
+// (hydro_stage_update.cuh) as kernel 2.  What changes is the eta_s axis, where the ncu profile of kernel 2 put 43 % of
+// the stall samples on 28 % of the instructions (profiles/round2_kernel2.md: the four off-centre planes of the
+// eta_s star miss L1, long-scoreboard stalls 2.3-3.2 warps per issue):
+//   * a block owns a 32 x 8 column of cells and walks through a chunk of eta_s planes;
+//   * the eta_s flux is a PIPELINE per column: when plane p comes into reach the limited slope of cell p-1 and the
+//     KT face p-3/2 are formed ONCE (kernel 2: every eta slope three times, every face twice), and the flux difference
+//     of cell k = p-2 is completed from the kept left state (Q^l, F^l) of cell p-2 and the kept face flux p-5/2;
+//   * that kept state -- 3 values for each of the 14 evolved fields -- is indexed at run time by the rolled pi-field
+//     loop, so it cannot sit in registers; it lives in TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32x32b: every thread
+//     owns a lane segment), which leaves the unified L1 / shared memory to the x and y stars.  No tensor-core
+//     instruction is issued;
+//   * per step only ONE new plane is touched (own column, prefetched into L1 one plane ahead); planes p-1 and p-2 were
+//     read one and two steps earlier.
+// Citations: KT scheme PAPER.md:193-213 (Eq.40-44); RK2 :225-239 (Eq.49-54).
+#pragma once
+#include "hydro_stage_fused.cuh"
+#include "hydro_stage_tile.cuh"      // PrivTmem, lr, face2
+
+namespace clv {
+
+#ifndef CLV_MARCH_PF
+#define CLV_MARCH_PF 1      // prefetch of the own column of plane p+1: 1 into L1, 2 into L2, 0 none
+#endif
+#ifndef CLV_MARCH_SYNC
+#define CLV_MARCH_SYNC 1    // block barrier per plane: keeps the warps of a block on the same instruction-cache lines
+                            // (measured at 301x301x201: 15.7 -> 13.4 ms per step fp64, 7.6 -> 6.95 fp32; "no instruction"
+                            // stalls 1.8 -> 0.19 warps per issue, profiles/round2_kernel4.md)
+#endif
+
+// columns of tensor memory a block allocates: 8 warps share 4 lane quadrants, 3 kept values per evolved field
+template <typename R>
+struct MarchTmem {
+  static constexpr int W = sizeof(R) / 4;
+  static constexpr int COLS_PER_THREAD = 14 * 3 * W;                      // 84 (fp64) / 42 (fp32)
+  static constexpr int ALLOC_COLS = 2 * COLS_PER_THREAD <= 128 ? 128 : 256;
+  unsigned base;
+  __device__ __forceinline__ void init(unsigned tmem_base, int warp) {
+    base = tmem_base + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)((warp >> 2) * COLS_PER_THREAD);
+  }
+  __device__ __forceinline__ void get(int f, R& ql, R& fl, R& h) const { tm_ld3(base + f * 3 * W, ql, fl, h); }
+  __device__ __forceinline__ void put(int f, R ql, R fl, R h) const {
+    tm_st(base + f * 3 * W, ql); tm_st(base + (f * 3 + 1) * W, fl); tm_st(base + (f * 3 + 2) * W, h);
+  }
+};
+
+template <typename R, bool VISC, int MODE>
+__global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> a, const int chunk) {
+  static_assert(MODE == 1 || MODE == 2, "the bootstrap (MODE 0) runs in the per-cell kernel");
+  constexpr bool USE_PI = VISC;
+  constexpr int NF = VISC ? 14 : 4;
+  constexpr int OX = NF * FS;
+  const int lane = threadIdx.x, row = threadIdx.y, tid = row * 32 + lane;
+  const int i = blockIdx.x * 32 + lane, j = blockIdx.y * 8 + row;
+  const bool active = (i < a.nx) && (j < a.ny);
+  const int ic = active ? i : 0, jc = active ? j : 0;
+  const int kc0 = blockIdx.z * chunk, kc1 = min(kc0 + chunk, a.nz);
+  constexpr int sf = FS;
+  const R* __restrict__ in = a.in;
+
+  __shared__ R sS[USE_PI ? 10 * 256 : 1];
+  __shared__ unsigned s_tmem;
+  using Priv = MarchTmem<R>;
+  if (row == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)),
+                 "r"((unsigned)Priv::ALLOC_COLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  Priv priv;
+  priv.init(s_tmem, row);
+
+  // in-plane offsets (elements) of the x and y stars and of the column itself
+  // (32-bit: hydro_create admits kernel 4 only when a plane has fewer than 2^31 elements)
+  const int col = (int)(jc * a.sy + xoff(ic, a.blk));
+  int offx[5], offy[5];
+#pragma unroll
+  for (int p = 0; p < 5; ++p) {
+    offx[p] = (int)(jc * a.sy + xoff(bmap(ic + p - 2, a.nx, a.bc[0]), a.blk));
+    offy[p] = (int)(bmap(jc + p - 2, a.ny, a.bc[1]) * a.sy + xoff(ic, a.blk));
+  }
+  const long long cg0 = (long long)jc * a.gp + ic;
+
+  const R tf = a.milne ? a.tau : R(1);
+  const R th2 = R(2) * a.theta;
+  const R sc_pi = R(0.5) * a.scale[2], sc_T = sc_pi * tf;
+  R cflm0 = R(0), cflm1 = R(0), cflm2 = R(0), emax = R(0);
+
+  for (int p = kc0; p <= kc1 + 1; ++p) {
+    const int k = p - 2;
+    const bool centre = p >= kc0 + 2;                      // block-uniform
+    if (CLV_MARCH_SYNC) __syncthreads();
+    const R* __restrict__ q2 = in + (long long)bmap(p - 2, a.nz, a.bc[2]) * a.sz + col;    // plane p-2 (= k)
+    const R* __restrict__ q1 = in + (long long)bmap(p - 1, a.nz, a.bc[2]) * a.sz + col;
+    const R* __restrict__ q0 = in + (long long)bmap(p, a.nz, a.bc[2]) * a.sz + col;
+    if (CLV_MARCH_PF && p + 1 <= kc1 + 1 && (lane & (sizeof(R) == 8 ? 15 : 31)) == 0) {
+      const R* __restrict__ qn = in + (long long)bmap(p + 1, a.nz, a.bc[2]) * a.sz + col;
+#pragma unroll
+      for (int m = 0; m < NF + X_COUNT; ++m) {
+        if (CLV_MARCH_PF == 1) prefetch_l1(qn + m * FS);
+        else asm volatile("prefetch.global.L2 [%0];" ::"l"(qn + m * FS));
+      }
+    }
+
+    R S[14];
+#pragma unroll
+    for (int m = 0; m < 14; ++m) S[m] = R(0);
+    R cfl2;
+    // ---- eta_s pipeline step: slope of cell p-1, face p-3/2, flux difference of cell p-2 ---------------------------
+    {
+      const R* __restrict__ pp[3] = {q2, q1, q0};
+      R g[3], ua[3];
+#pragma unroll
+      for (int t = 0; t < 3; ++t) { g[t] = pp[t][OX + X_G * FS]; ua[t] = pp[t][3 * FS]; }
+      const R c2 = q2[OX + X_CN * FS];
+      const R cface = max_(c2, q1[OX + X_CN * FS]);
+      cfl2 = c2 * a.h * a.scale[2];
+      {
+        R wq[3], wa[3], Pp[3];
+#pragma unroll
+        for (int t = 0; t < 3; ++t) {
+          Pp[t] = pp[t][OX + X_P * FS];
+          const R w = pp[t][0] + Pp[t];
+          wq[t] = w * g[t]; wa[t] = w * ua[t];
+        }
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+          R q[3], f[3];
+          const int o_t = (F_PI + mu) * FS, o_a = (F_PI + c_pidx[3][mu]) * FS;
+#pragma unroll
+          for (int t = 0; t < 3; ++t) {
+            const R umu = mu == 0 ? g[t] : pp[t][mu * FS];
+            R tq = wq[t] * umu - (mu == 0 ? Pp[t] : R(0));
+            R tfl = wa[t] * umu + (mu == 3 ? Pp[t] : R(0));
+            if (USE_PI) { tq += pp[t][o_t]; tfl += pp[t][o_a]; }
+            q[t] = tq; f[t] = tfl;
+          }
+          R QLk, FLk, Hk, QL1, QR1, FL1, FR1;
+          priv.get(mu, QLk, FLk, Hk);
+          lr(q[0], q[1], q[2], th2, QL1, QR1);
+          lr(f[0], f[1], f[2], th2, FL1, FR1);
+          const R Hn = face2(QLk, FLk, QR1, FR1, cface);
+          S[mu] = -(Hn - Hk) * sc_T;
+          priv.put(mu, QL1, FL1, Hn);
+        }
+      }
+      if (USE_PI) {
+        R* slot = &sS[tid];
+#pragma unroll 1
+        for (int t = 0; t < 5; ++t) {
+          const int fa = F_PI + 2 * t;
+          R QLa, FLa, Ha, QLb, FLb, Hb;
+          priv.get(fa, QLa, FLa, Ha);
+          priv.get(fa + 1, QLb, FLb, Hb);
+          R qa[3], fa_[3], qb[3], fb[3];
+#pragma unroll
+          for (int s = 0; s < 3; ++s) {
+            const R va = pp[s][fa * FS], vb = pp[s][(fa + 1) * FS];
+            qa[s] = g[s] * va; fa_[s] = ua[s] * va;
+            qb[s] = g[s] * vb; fb[s] = ua[s] * vb;
+          }
+          R QL1, QR1, FL1, FR1;
+          lr(qa[0], qa[1], qa[2], th2, QL1, QR1);
+          lr(fa_[0], fa_[1], fa_[2], th2, FL1, FR1);
+          const R Hna = face2(QLa, FLa, QR1, FR1, cface);
+          priv.put(fa, QL1, FL1, Hna);
+          lr(qb[0], qb[1], qb[2], th2, QL1, QR1);
+          lr(fb[0], fb[1], fb[2], th2, FL1, FR1);
+          const R Hnb = face2(QLb, FLb, QR1, FR1, cface);
+          priv.put(fa + 1, QL1, FL1, Hnb);
+          slot[0] = -(Hna - Ha) * sc_pi;
+          slot[256] = -(Hnb - Hb) * sc_pi;
+          slot += 2 * 256;
+        }
+      }
+      tm_wait_st();
+    }
+    if (!centre) continue;
+
+    // ---- x and y flux differences of cell k (five-point stars inside plane k) ---------------------------------------
+    const R* __restrict__ plane = in + (long long)bmap(k, a.nz, a.bc[2]) * a.sz;
+    const R* __restrict__ pc = plane + col;
+    R cfl0, cfl1;
+    {
+      const R* __restrict__ pp[5];
+#pragma unroll
+      for (int t = 0; t < 5; ++t) pp[t] = plane + offx[t];
+      axis_flux<R, USE_PI, 0, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl0);
+#pragma unroll
+      for (int t = 0; t < 5; ++t) pp[t] = plane + offy[t];
+      axis_flux<R, USE_PI, 1, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl1);
+    }
+    if (USE_PI) {
+#pragma unroll
+      for (int m = 0; m < 10; ++m) S[4 + m] = sS[m * 256 + tid];
+    }
+
+    // ---- cell-centre state, velocity gradients ------------------------------------------------------------------------
+    Cell<R> cc, cn_;
+    cc.e = pc[0];
+    cc.u[1] = pc[sf]; cc.u[2] = pc[2 * sf]; cc.u[3] = pc[3 * sf];
+    cc.u[0] = pc[OX + X_G * FS];
+    cc.P = pc[OX + X_P * FS];
+#pragma unroll
+    for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
+    R grad[4][4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m)
+#pragma unroll
+      for (int n = 0; n < 4; ++n) grad[m][n] = R(0);
+    if (USE_PI) {
+      const R* __restrict__ zm = in + (long long)bmap(k - 1, a.nz, a.bc[2]) * a.sz + col;
+#pragma unroll
+      for (int ax = 0; ax < 3; ++ax) {
+        const R* __restrict__ qm = ax == 0 ? plane + offx[1] : (ax == 1 ? plane + offy[1] : zm);
+        const R* __restrict__ qp = ax == 0 ? plane + offx[3] : (ax == 1 ? plane + offy[3] : q1);
+        const R sc = R(0.5) * a.scale[ax];
+        grad[ax + 1][0] = (qp[OX + X_G * FS] - qm[OX + X_G * FS]) * sc;
+        grad[ax + 1][1] = (qp[sf] - qm[sf]) * sc;
+        grad[ax + 1][2] = (qp[2 * sf] - qm[2 * sf]) * sc;
+        grad[ax + 1][3] = (qp[3 * sf] - qm[3 * sf]) * sc;
+      }
+    }
+    const long long c = (long long)k * a.sz + col;
+    const long long cg = (long long)k * a.ny * a.gp + cg0;
+    if (MODE == 2) {
+      const R* __restrict__ sn = a.sn + c;
+      cn_.e = sn[0];
+      cn_.u[1] = sn[sf]; cn_.u[2] = sn[2 * sf]; cn_.u[3] = sn[3 * sf];
+      cn_.u[0] = sn[OX + X_G * FS];
+      cn_.P = sn[OX + X_P * FS];
+#pragma unroll
+      for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
+    }
+    R up3[3] = {R(0), R(0), R(0)};
+    R gst = R(1);
+    if (USE_PI) {
+      if (MODE == 1) {
+        const R* __restrict__ up = a.uprev + c;
+        up3[0] = up[0]; up3[1] = up[sf]; up3[2] = up[2 * sf];
+      } else {
+        gst = a.gstar[cg];
+      }
+    }
+
+    // ---- sources, stage update, root-find, limiter (hydro_stage_update.cuh) -----------------------------------------
+    unsigned flags = 0;
+    Cell<R> nw;
+    R cs2_new;
+    stage_update<R, VISC, MODE>(a, S, cc, cn_, grad, up3, gst, nw, cs2_new, flags);
+
+    if (active) {
+      R* __restrict__ out = a.out + c;
+      R cx, cy, cn;
+      signal_speeds3(nw.u[0], nw.u[1], nw.u[2], nw.u[3], cs2_new, cx, cy, cn);
+      out[0] = nw.e; out[sf] = nw.u[1]; out[2 * sf] = nw.u[2]; out[3 * sf] = nw.u[3];
+      if (VISC) {
+#pragma unroll
+        for (int m = 0; m < 10; ++m) out[(F_PI + m) * FS] = nw.pi[m];
+        if (MODE == 1) a.gstar[cg] = gst;
+      }
+      out[OX + X_P * FS] = nw.P; out[OX + X_G * FS] = nw.u[0];
+      out[OX + X_CX * FS] = cx; out[OX + X_CY * FS] = cy; out[OX + X_CN * FS] = cn;
+      if (MODE == 1) { cflm0 = max_(cflm0, cfl0); cflm1 = max_(cflm1, cfl1); cflm2 = max_(cflm2, cfl2); }
+      else emax = max_(emax, nw.e);
+    } else {
+      flags = 0;
+    }
+    count_flags(a.diag, flags);
+  }
+
+  // the tensor memory goes back (the warp that allocated it frees it; every thread has waited on its accesses)
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (row == 0) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(s_tmem), "r"((unsigned)Priv::ALLOC_COLS)
+                 : "memory");
+  }
+
+  // ---- reductions (row a10): one atomic per warp per block ------------------------------------------------------------
+  if (MODE == 1) {
+    const double r0 = warp_max((double)cflm0), r1 = warp_max((double)cflm1), r2 = warp_max((double)cflm2);
+    if (lane == 0) {
+      atomic_max_nonneg(&a.diag->cfl[a.slot][0], r0);
+      atomic_max_nonneg(&a.diag->cfl[a.slot][1], r1);
+      atomic_max_nonneg(&a.diag->cfl[a.slot][2], r2);
+    }
+  } else {
+    const double r = warp_max((double)emax);
+    if (lane == 0) atomic_max_nonneg(&a.diag->emax[a.slot], r);
+  }
+  if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && tid == 0) {
+    if (MODE == 1) a.diag->emax[a.slot] = 0ull;
+    else { a.diag->cfl[a.slot ^ 1][0] = 0ull; a.diag->cfl[a.slot ^ 1][1] = 0ull; a.diag->cfl[a.slot ^ 1][2] = 0ull; }
+  }
+}
+
+// planes per chunk: whole waves of the 2-blocks-per-SM residency, against the two pipeline warm-up planes of a chunk
+inline int march_chunk(int nx, int ny, int nz, int nsm) {
+  const long long tiles = (long long)((nx + 31) / 32) * ((ny + 7) / 8);
+  const long long slots = 2ll * nsm;
+  double best = -1.0;
+  int best_chunk = nz;
+  for (int nchunk = 1; nchunk <= nz; ++nchunk) {
+    const int chunk = (nz + nchunk - 1) / nchunk;
+    const long long blocks = tiles * ((nz + chunk - 1) / chunk);
+    const long long waves = (blocks + slots - 1) / slots;
+    const double eff = (double)blocks / (double)(waves * slots) * (double)chunk / ((double)chunk + 0.6);
+    if (eff > best * 1.0001) { best = eff; best_chunk = chunk; }
+  }
+  return best_chunk;
+}
+
+template <typename R, bool VISC, int MODE>
+void launch_stage_march(const StageArgs<R>& a, int chunk, cudaStream_t stream) {
+  dim3 block(32, 8, 1);
+  dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, (a.nz + chunk - 1) / chunk);
+  stage_march_kernel<R, VISC, MODE><<<grid, block, 0, stream>>>(a, chunk);
+}
+
+}  // namespace clv

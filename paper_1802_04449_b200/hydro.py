@@ -15,7 +15,8 @@ from . import build as _build
 
 HYDRO_MEM_DEVICE, HYDRO_MEM_HOST = 0, 1
 SYMBOLS = ["hydro_workspace_bytes", "hydro_create", "hydro_load", "hydro_set_history", "hydro_read_history",
-           "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_kernel", "hydro_destroy", "hydro_strerror"]
+           "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_kernel", "hydro_destroy", "hydro_strerror",
+           "hydro_freezeout_bytes", "hydro_freezeout_begin", "hydro_freezeout_slab", "hydro_freezeout_run"]
 
 
 class hydro_grid(Structure):
@@ -72,6 +73,16 @@ def load_library():
     lib.hydro_launch_count.argtypes = [c_void_p]
     lib.hydro_kernel.restype = c_int
     lib.hydro_kernel.argtypes = [c_void_p]
+    lib.hydro_freezeout_bytes.restype = c_size_t
+    lib.hydro_freezeout_bytes.argtypes = [POINTER(hydro_grid), c_int]
+    lib.hydro_freezeout_begin.restype = c_int
+    lib.hydro_freezeout_begin.argtypes = [c_void_p, c_void_p, c_size_t, c_double]
+    lib.hydro_freezeout_slab.restype = c_int
+    lib.hydro_freezeout_slab.argtypes = [c_void_p, c_void_p, c_void_p, c_longlong, POINTER(c_longlong),
+                                         POINTER(c_longlong)]
+    lib.hydro_freezeout_run.restype = c_int
+    lib.hydro_freezeout_run.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_longlong, POINTER(c_longlong),
+                                        POINTER(c_int)]
     lib.hydro_destroy.restype = None
     lib.hydro_destroy.argtypes = [c_void_p]
     lib.hydro_strerror.restype = ctypes.c_char_p
@@ -222,11 +233,52 @@ class Hydro:
                     clamped=int(d.n_clamp), pi_limited=int(d.n_pi_limited), nan=int(d.n_nan),
                     root_unconverged=int(d.n_root_unconverged), warn=warn)
 
+    # -- freeze-out hypersurface -------------------------------------------------
+    def freezeout_begin(self, e_frz, capacity):
+        """Store the current state as level a; allocate the finder's workspace and the element arrays (device)."""
+        torch = self._torch
+        with torch.cuda.device(self.device):
+            nbytes = int(self._lib.hydro_freezeout_bytes(byref(self.grid), self.precision))
+            self._frz_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._frz_ws.data_ptr() + 255) // 256 * 256
+            self._frz_keys = torch.empty(capacity, dtype=torch.int64, device=self.device)
+            self._frz_rows = torch.empty((capacity, 22), dtype=torch.float64, device=self.device)
+            self._frz_cap, self._frz_n = int(capacity), 0
+            _check(self._lib.hydro_freezeout_begin(self._h, c_void_p(base), nbytes, float(e_frz)),
+                   "hydro_freezeout_begin")
+
+    def freezeout_slab(self):
+        """Append the elements between the stored level and the current state; returns (n_total, n_hot)."""
+        n, hot = c_longlong(0), c_longlong(0)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_freezeout_slab(self._h, c_void_p(self._frz_keys.data_ptr()),
+                                                  c_void_p(self._frz_rows.data_ptr()), self._frz_cap, byref(n),
+                                                  byref(hot)), "hydro_freezeout_slab")
+        self._frz_n = int(n.value)
+        return self._frz_n, int(hot.value)
+
+    def freezeout_run(self, steps_per_slab, max_slabs):
+        """{step(steps_per_slab); slab} until no cell is hotter than e_frz or max_slabs; returns
+        (n_total, slabs done)."""
+        n, ns = c_longlong(0), c_int(0)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_freezeout_run(self._h, int(steps_per_slab), int(max_slabs),
+                                                 c_void_p(self._frz_keys.data_ptr()),
+                                                 c_void_p(self._frz_rows.data_ptr()), self._frz_cap, byref(n),
+                                                 byref(ns)), "hydro_freezeout_run")
+        self._frz_n = int(n.value)
+        return self._frz_n, int(ns.value)
+
+    def freezeout_elements(self):
+        """(keys int64 [M], rows float64 [M, 22]) gathered so far, as CUDA tensors in emission order."""
+        return self._frz_keys[:self._frz_n], self._frz_rows[:self._frz_n]
+
     def launch_count(self) -> int:
         return int(self._lib.hydro_launch_count(self._h))
 
     def kernel(self) -> int:
-        """The stage kernel in use (1 reference, 2 per-cell fused, 3 tile); kernel=0 resolves to the fastest measured (2)."""
+        """The stage kernel in use (1 reference, 2 per-cell fused, 3 tile, 4 marching per-cell); kernel=0 resolves to the
+        fastest measured (4)."""
         return int(self._lib.hydro_kernel(self._h))
 
     def close(self):

@@ -21,7 +21,7 @@ def test_full_size_first_steps(crossover, which, steps):
     o.step(steps)
     ref = o.read()
     do = o.diag()
-    for kernel in (2, 3):                       # both production kernels, fp64
+    for kernel in (2, 3, 4):                       # both production kernels, fp64
         g = from_config(cfg, crossover, kernel=kernel)
         g.load(T)
         g.step(steps)
@@ -33,7 +33,7 @@ def test_full_size_first_steps(crossover, which, steps):
         assert np.allclose(dg["cfl"], do["cfl"], rtol=1e-9) and abs(dg["e_max"] / do["e_max"] - 1) < 1e-10
         assert dg["nan"] == 0 and dg["root_unconverged"] == 0
         del g
-    for kernel in (2, 3):
+    for kernel in (2, 3, 4):
         g32 = from_config(cfg, crossover, precision=32, kernel=kernel)
         g32.load(T.astype(np.float32))
         g32.step(steps)
@@ -43,7 +43,7 @@ def test_full_size_first_steps(crossover, which, steps):
         del g32
 
 
-@pytest.mark.parametrize("kernel", [2, 3])
+@pytest.mark.parametrize("kernel", [2, 3, 4])
 @pytest.mark.parametrize("eta_s", [0.0, 0.2])
 def test_gubser_on_gpu(conformal, eta_s, kernel):
     """configs[1]b at the stated resolution (201x201x1, dx = 0.05) from tau = 1 to 1.5 on the GPU, against the
@@ -77,7 +77,7 @@ def test_gubser_on_gpu(conformal, eta_s, kernel):
         assert np.all(np.abs(p[[3, 6, 8]]) < 1e-12) and np.all(np.abs(u[3]) < 1e-12)
 
 
-@pytest.mark.parametrize("kernel", [1, 2, 3])
+@pytest.mark.parametrize("kernel", [1, 2, 3, 4])
 def test_gubser_lambda1_on_gpu(conformal, kernel):
     """SURVEY 8(f)-2 on the GPU: the lambda_1 term and the free tau_pi coefficient against the paper's closed-form
     Gubser solution and against the oracle on the same grid."""

@@ -16,7 +16,7 @@ from parity_util import errors, make_oracle
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("kernel", [2, 3])
+@pytest.mark.parametrize("kernel", [2, 3, 4])
 @pytest.mark.parametrize("which,precision", [("cfg2", 64), ("cfg2", 32), ("cfg3", 64), ("cfg3", 32), ("cfg4", 64),
                                              ("cfg4", 32)])
 def test_full_length_stability(crossover, which, precision, kernel):
@@ -60,7 +60,7 @@ def test_static_event_100_steps(crossover):
     cfg = sub_box(False)
     T, _ = inputs.ic_partons(cfg, inputs.seed_for(2))
     o = make_oracle(cfg, crossover); o.load(T)
-    gs = {(k, pr): from_config(cfg, crossover, precision=pr, kernel=k) for k in (2, 3) for pr in (64, 32)}
+    gs = {(k, pr): from_config(cfg, crossover, precision=pr, kernel=k) for k in (2, 3, 4) for pr in (64, 32)}
     for g in gs.values():
         g.load(T.astype(g.np_dtype))
     for s in (25, 50, 100):
@@ -78,7 +78,7 @@ def test_static_event_100_steps(crossover):
     assert o.diag()["clamped"] == 0 and all(g.diag()["clamped"] == 0 for g in gs.values())
 
 
-@pytest.mark.parametrize("kernel", [2, 3])
+@pytest.mark.parametrize("kernel", [2, 3, 4])
 def test_moving_event_drift_is_rounding_chaos(crossover, kernel):
     """96x96x64 sub-box of configs[3] (moving partons, eta/s = 0.08).  The rim is clamped to gamma = 22.4 within 25
     steps; from then on ANY two roundings of the algorithm drift apart.  Measured (B200, round 2), L2(e) over
@@ -116,7 +116,7 @@ def test_moving_event_drift_is_rounding_chaos(crossover, kernel):
         assert abs(ncg - nco) <= 0.05 * nco + 10
 
 
-@pytest.mark.parametrize("kernel", [2, 3])
+@pytest.mark.parametrize("kernel", [2, 3, 4])
 @pytest.mark.parametrize("eta_s", [0.0, 0.08, 0.2])
 def test_bjorken_on_gpu_to_tau10(conformal, eta_s, kernel):
     """configs[1]a on the GPU: 1x1x1 periodic cell, e(0.6) = 30, tau 0.6 -> 10 with h = 0.01 (940 steps), against the

@@ -11,7 +11,7 @@ from parity_util import errors, make_oracle, small_parton_config
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [1, 2, 3]
+KERNELS = [1, 2, 3, 4]
 
 
 def gpu(cfg, eos, **kw):
