@@ -92,6 +92,10 @@ typedef struct {
    * the relaxation time tau_pi = tau_pi_coeff eta_v/(T s), <= 0 selects the paper's 5.  The paper's
    * closed-form Gubser test uses lambda1_hat = -10 and tau_pi_coeff = 4 lambda1_hat^2 / 9. */
   double lambda1_hat, tau_pi_coeff;
+  /* SURVEY 8(f)-4 (Eq.53 as printed; A12): 1 = the stage-2 right-hand side of T^{tau mu} is
+   * evaluated with pi^{n+1} (the result of Eq.52) instead of pi': stage 2 becomes three launches (4 per RK2 step).
+   * Kernels 2 and 4 only (HYDRO_EINVAL otherwise); ignored for eta_over_s = 0.  0 = standard Heun (default). */
+  int strict_eq53;
 } hydro_opts;
 
 /* Diagnostics (PAPER.md:640 for e_max).  cfl[a] = max over cells of

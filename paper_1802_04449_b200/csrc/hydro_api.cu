@@ -29,6 +29,7 @@
 #include "hydro_stage_tile.cuh"
 #include "hydro_stage_march.cuh"
 #include "hydro_freezeout.cuh"
+#include "hydro_stage_strict.cuh"
 
 namespace clv {
 
@@ -49,7 +50,7 @@ struct Layout {
 };
 
 // kernel 0 = the fastest one as measured on B200 at 301x301x201 (round 2): the marching per-cell
-// kernel (4) in both precisions: fp64 13.4 ms per step against 14.4 (kernel 2) and 15.7 (kernel 3); fp32 6.95 against
+// kernel (4) in both precisions: fp64 11.8 ms per step against 14.4 (kernel 2) and 15.7 (kernel 3); fp32 6.3 against
 // 7.5 and 8.0.
 static int resolve_kernel(int kernel, int precision) { (void)precision; return kernel != 0 ? kernel : 4; }
 
@@ -276,7 +277,7 @@ using namespace clv;
 struct hydro_ctx {
   hydro_grid grid;
   double dtau, tau0, eta_s;
-  int precision, visc, kernel;
+  int precision, visc, kernel, strict;
   double theta, e_floor, xi, v_max, lambda1_hat, c_tau;
   int root_iters;
   Layout L;
@@ -472,7 +473,10 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
 template <typename R, bool VISC, int MODE>
 int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
   if (c->kernel == 4 && MODE != 0) {
-    if constexpr (MODE != 0) launch_stage_march<R, VISC, MODE>(a, c->march_chunk, c->stream);
+    if constexpr (MODE != 0) {
+      c->launches += 1;
+      return launch_stage_march<R, VISC, MODE>(a, c->march_chunk, c->stream) == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+    }
   } else if (c->kernel == 2 || c->kernel == 4) {      // the bootstrap of kernel 4 runs in the per-cell kernel (same store)
     launch_stage_fused<R, VISC, MODE>(a, c->stream);
   } else {
@@ -531,7 +535,22 @@ int do_step(hydro_ctx* c) {
   StageArgs<R> a2 = stage_args<R>(c, tau_1, tau_n, tau_1);
   a2.in = X; a2.sn = cur; a2.gstar = static_cast<R*>(c->gstar); a2.out = prev; a2.slot = slot;
   int rc;
-  if (c->visc) {
+  if (c->visc && c->strict) {
+    // Eq.53 as printed (A12; hydro_stage_strict.cuh): sweep A = stage 2 without limiter into a scratch diag block,
+    // sweep B = T fields on (e', u', pi^{n+1}), sweep C = limiter
+    rc = launch_stage<R, true, 1>(c, a1);
+    if (rc) return rc;
+    StageArgs<R> a2a = a2;
+    a2a.xi = R(0); a2a.diag = c->diag + 1;
+    rc = launch_stage<R, true, 2>(c, a2a);
+    if (rc) return rc;
+    dim3 block(32, 8, 1);
+    dim3 grid((a2.nx + 31) / 32, (a2.ny + 7) / 8, a2.nz);
+    stage_strict_T_kernel<R><<<grid, block, 0, c->stream>>>(a2, prev);
+    stage_strict_limit_kernel<R><<<grid, block, 0, c->stream>>>(a2);
+    c->launches += 2;
+    rc = cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+  } else if (c->visc) {
     rc = launch_stage<R, true, 1>(c, a1);
     if (rc) return rc;
     rc = launch_stage<R, true, 2>(c, a2);
@@ -688,6 +707,10 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   if (!grid || !eos || !opts) return HYDRO_EINVAL;
   Layout L;
   if (opts->kernel < 0 || opts->kernel > 4) return HYDRO_EINVAL;
+  if (opts->strict_eq53 && eta_over_s > 0.0) {      // the strict sweeps exist for the blocked extended store only
+    const int kk = resolve_kernel(opts->kernel, opts->precision);
+    if (kk != 2 && kk != 4) return HYDRO_EINVAL;
+  }
   if (!make_layout(grid, opts->precision, eta_over_s, opts->kernel, &L)) return HYDRO_EINVAL;
   if (!(dtau > 0.0) || !(grid->dx > 0.0) || !(grid->dy > 0.0) || !(grid->deta > 0.0)) return HYDRO_EINVAL;
   if (grid->geometry != 0 && grid->geometry != 1) return HYDRO_EINVAL;
@@ -715,6 +738,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->grid = *grid; c->dtau = dtau; c->tau0 = tau0; c->eta_s = eta_over_s;
   c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
   c->kernel = resolve_kernel(opts->kernel, opts->precision);
+  c->strict = opts->strict_eq53 ? 1 : 0;
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
   c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;
@@ -734,7 +758,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
     int dev = 0, nsm = 148;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
       rc = HYDRO_ECUDA;
-    c->march_chunk = march_chunk(grid->nx, grid->ny, grid->nz, nsm > 0 ? nsm : 148);
+    c->march_chunk = march_chunk(grid->nx, grid->ny, grid->nz, nsm > 0 ? nsm : 148, opts->precision == 64 ? 2 : CLV_MARCH_MINB32);
   }
   if (rc == HYDRO_OK && L.soa) {
     int dev = 0, nsm = 148;

@@ -147,17 +147,18 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // KT flux difference (Eq.40-44) of every evolved field along axis AX from the five-point star pp[0..4] of the extended
 // state (pp[2] = the cell itself).  T fields: S[0..3] -= ...; pi fields: the thread-private shared-memory slots
 // slot0[m * 256] (INIT: first axis, "=" instead of "-=").  cfl = c_a h / Delta_a of the cell.  Shared by the per-cell
-// kernel (three axes) and the marching kernel (x and y; hydro_stage_march.cuh).
-template <typename R, bool USE_PI, int AX, bool INIT, int OX, typename A>
+// kernel (three axes) and the marching kernel (x and y; hydro_stage_march.cuh).  FSTR = element stride between the
+// fields of a point (32 in the blocked global store; the plane size of a shared-memory tile).
+template <typename R, bool USE_PI, int AX, bool INIT, int OX, int FSTR = FS, typename A>
 __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ const (&pp)[5], R th2, R tf, R (&S)[14],
                                           R* slot0, R& cfl) {
-  const int o_ua = (1 + AX) * FS, o_ca = OX + (X_CX + AX) * FS;
+  const int o_ua = (1 + AX) * FSTR, o_ca = OX + (X_CX + AX) * FSTR;
   if (CLV_PFZ && USE_PI && AX == 2) {      // first pi trip of this axis: in flight behind the T-field part
 #pragma unroll
     for (int p = 0; p < 5; ++p)
       if (p != 2) {
 #pragma unroll
-        for (int m = 0; m < 2 * CLV_PFD; ++m) prefetch_l1(pp[p] + (F_PI + m) * FS);
+        for (int m = 0; m < 2 * CLV_PFD; ++m) prefetch_l1(pp[p] + (F_PI + m) * FSTR);
       }
   }
 
@@ -169,7 +170,7 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
     cfl = c2 * a.h * a.scale[AX];
   }
 #pragma unroll
-  for (int p = 0; p < 5; ++p) { g[p] = pp[p][OX + X_G * FS]; ua[p] = pp[p][o_ua]; }
+  for (int p = 0; p < 5; ++p) { g[p] = pp[p][OX + X_G * FSTR]; ua[p] = pp[p][o_ua]; }
   const R sc_pi = R(0.5) * a.scale[AX], sc_T = sc_pi * tf;
 
   {
@@ -177,7 +178,7 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
     R wq[5], wa[5], Pp[5];
 #pragma unroll
     for (int p = 0; p < 5; ++p) {
-      Pp[p] = pp[p][OX + X_P * FS];
+      Pp[p] = pp[p][OX + X_P * FSTR];
       const R w = pp[p][0] + Pp[p];
       wq[p] = w * g[p]; wa[p] = w * ua[p];
     }
@@ -186,12 +187,12 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
 #pragma unroll
       for (int hp = 0; hp < 2; ++hp) {
         const int m0 = 2 * hp, m1 = m0 + 1;
-        const int o_t0 = (F_PI + m0) * FS, o_t1 = (F_PI + m1) * FS;
-        const int o_a0 = (F_PI + c_pidx[AX + 1][m0]) * FS, o_a1 = (F_PI + c_pidx[AX + 1][m1]) * FS;
+        const int o_t0 = (F_PI + m0) * FSTR, o_t1 = (F_PI + m1) * FSTR;
+        const int o_a0 = (F_PI + c_pidx[AX + 1][m0]) * FSTR, o_a1 = (F_PI + c_pidx[AX + 1][m1]) * FSTR;
         F2 q[5], f[5];
 #pragma unroll
         for (int p = 0; p < 5; ++p) {
-          const F2 um = {m0 == 0 ? (float)g[p] : (float)pp[p][m0 * FS], (float)pp[p][m1 * FS]};
+          const F2 um = {m0 == 0 ? (float)g[p] : (float)pp[p][m0 * FSTR], (float)pp[p][m1 * FSTR]};
           F2 cq = {m0 == 0 ? -(float)Pp[p] : 0.0f, 0.0f};
           F2 cf = {m0 == AX + 1 ? (float)Pp[p] : 0.0f, m1 == AX + 1 ? (float)Pp[p] : 0.0f};
           if (USE_PI) {
@@ -207,12 +208,12 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
       R q[5], f[5];
-      const int o_t = (F_PI + (mu == 0 ? 0 : mu)) * FS;            // pi^{tau mu}: components 0..3
-      const int o_a = (F_PI + c_pidx[AX + 1][mu]) * FS;            // pi^{a mu} (a constant-memory lookup measured
+      const int o_t = (F_PI + (mu == 0 ? 0 : mu)) * FSTR;            // pi^{tau mu}: components 0..3
+      const int o_a = (F_PI + c_pidx[AX + 1][mu]) * FSTR;            // pi^{a mu} (a constant-memory lookup measured
                                                                    // faster than a constexpr index here)
 #pragma unroll
       for (int p = 0; p < 5; ++p) {
-        const R umu = mu == 0 ? g[p] : pp[p][mu * FS];
+        const R umu = mu == 0 ? g[p] : pp[p][mu * FSTR];
         R tq = wq[p] * umu - (mu == 0 ? Pp[p] : R(0));
         R tfl = wa[p] * umu + (mu == AX + 1 ? Pp[p] : R(0));
         if (USE_PI) { tq += pp[p][o_t]; tfl += pp[p][o_a]; }
@@ -228,7 +229,7 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
     // offsets inside a trip are immediates and the five star pointers are bumped once per trip
     const R* __restrict__ pq[5];
 #pragma unroll
-    for (int p = 0; p < 5; ++p) pq[p] = pp[p] + F_PI * FS;
+    for (int p = 0; p < 5; ++p) pq[p] = pp[p] + F_PI * FSTR;
     R* slot = slot0;
     if constexpr (CLV_PACK32 && sizeof(R) == 4) {
       F2 g2[5], ua2[5];
@@ -241,13 +242,13 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
         if (CLV_PFZ && AX == 2) {
 #pragma unroll
           for (int p = 0; p < 5; ++p)
-            if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
+            if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FSTR); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FSTR); }
         }
 #pragma unroll
         for (int p = 0; p < 5; ++p) {
-          const F2 v = {(float)pq[p][0], (float)pq[p][FS]};
+          const F2 v = {(float)pq[p][0], (float)pq[p][FSTR]};
           q[p] = mul2(g2[p], v); f[p] = mul2(ua2[p], v);
-          pq[p] += 2 * FS;
+          pq[p] += 2 * FSTR;
         }
         const F2 d = kt_div2_2(q, f, cl2, ncr2, th22);
         const R da = R(d.x) * sc_pi, db = R(d.y) * sc_pi;
@@ -262,14 +263,14 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
       if (CLV_PFZ && AX == 2) {      // next trip's fields on the four off-centre planes
 #pragma unroll
         for (int p = 0; p < 5; ++p)
-          if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FS); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FS); }
+          if (p != 2) { prefetch_l1(pq[p] + CLV_PFD * 2 * FSTR); prefetch_l1(pq[p] + (CLV_PFD * 2 + 1) * FSTR); }
       }
 #pragma unroll
       for (int p = 0; p < 5; ++p) {
-        const R va = pq[p][0], vb = pq[p][FS];
+        const R va = pq[p][0], vb = pq[p][FSTR];
         qa[p] = g[p] * va; fa[p] = ua[p] * va;
         qb[p] = g[p] * vb; fb[p] = ua[p] * vb;
-        pq[p] += 2 * FS;
+        pq[p] += 2 * FSTR;
       }
       const R da = kt_div2(qa, fa, cl, cr, th2) * sc_pi;
       const R db = kt_div2(qb, fb, cl, cr, th2) * sc_pi;

@@ -1,19 +1,23 @@
-// hydro_stage_march.cuh -- "kernel 4": the per-cell fused stage kernel MARCHING along eta_s.
+// hydro_stage_march.cuh -- "kernel 4": the per-cell fused stage kernel MARCHING along eta_s (default kernel).
 //
 // Same field store (blocked extended state, 19 words per cell), same x / y flux code (axis_flux) and same stage tail
-// (hydro_stage_update.cuh) as kernel 2.  What changes is the eta_s axis, where the ncu profile of kernel 2 put 43 % of
-// the stall samples on 28 % of the instructions (profiles/round2_kernel2.md: the four off-centre planes of the
-// eta_s star miss L1, long-scoreboard stalls 2.3-3.2 warps per issue):
+// (hydro_stage_update.cuh) as kernel 2.  What changes follows the ncu profile of kernel 2 (profiles/round2_kernels.md:
+// 43 % of the stall samples on the 28 % of the instructions that form the eta_s fluxes, because the four off-centre
+// planes of the eta_s star miss L1; long-scoreboard stalls 2.3-3.2 warps per issue, L1 hit rate 53 %):
 //   * a block owns a 32 x 8 column of cells and walks through a chunk of eta_s planes;
 //   * the eta_s flux is a PIPELINE per column: when plane p comes into reach the limited slope of cell p-1 and the
 //     KT face p-3/2 are formed ONCE (kernel 2: every eta slope three times, every face twice), and the flux difference
 //     of cell k = p-2 is completed from the kept left state (Q^l, F^l) of cell p-2 and the kept face flux p-5/2;
 //   * that kept state -- 3 values for each of the 14 evolved fields -- is indexed at run time by the rolled pi-field
 //     loop, so it cannot sit in registers; it lives in TENSOR MEMORY (tcgen05.st / tcgen05.ld, 32x32b: every thread
-//     owns a lane segment), which leaves the unified L1 / shared memory to the x and y stars.  No tensor-core
-//     instruction is issued;
-//   * per step only ONE new plane is touched (own column, prefetched into L1 one plane ahead); planes p-1 and p-2 were
-//     read one and two steps earlier.
+//     owns a lane segment).  No tensor-core instruction is issued;
+//   * the x and y stars of plane k (and the cell's own state) are read from a SHARED-MEMORY TILE: 36 x 12 points x 19
+//     fields (65.7 KB fp64, two blocks per SM), filled with cp.async one plane ahead, behind the stage tail of the
+//     previous plane -- the paper's local-memory block, which its GPU had no room for.  The
+//     boundary rule a11 is applied to the source index of the copy, so the tile needs no special cases;
+//   * one block barrier per plane (two with the tile) keeps the 8 warps of a block on the same instruction-cache lines
+//     of the ~90 KB loop body: without it "no instruction" stalls are 1.8 warps per issue, with it 0.19.
+// Measured at 301x301x201 (profiles/round2_bench.md): 11.8 ms per step fp64, 6.3 ms fp32 (kernel 2: 14.4 / 7.5).
 // Citations: KT scheme PAPER.md:193-213 (Eq.40-44); RK2 :225-239 (Eq.49-54).
 #pragma once
 #include "hydro_stage_fused.cuh"
@@ -29,6 +33,27 @@ namespace clv {
                             // (measured at 301x301x201: 15.7 -> 13.4 ms per step fp64, 7.6 -> 6.95 fp32; "no instruction"
                             // stalls 1.8 -> 0.19 warps per issue, profiles/round2_kernel4.md)
 #endif
+
+#ifndef CLV_MARCH_TILE
+#define CLV_MARCH_TILE 1    // 1: the x / y stars of plane k are read from a shared-memory tile (32 x 8 cells + 2-cell halo,
+                            // all fields) filled with cp.async one plane ahead, behind the stage tail of the previous plane
+#endif
+#ifndef CLV_MARCH_ETA_TILE
+#define CLV_MARCH_ETA_TILE 1   // with the tile: the eta_s step takes plane p-2 (own column) from the tile too, so the tile
+                               // is also filled for the two warm-up planes of a chunk
+#endif
+#ifndef CLV_MARCH_PF_TAIL
+#define CLV_MARCH_PF_TAIL 0    // 1: L1 prefetch of what the stage tail reads at the cell (state n / history / u*^tau / plane
+                               // k-1); measured neutral (11.84 vs 11.75 ms fp64), off
+#endif
+constexpr int MT_SX = 36, MT_SY = 12, MT_FST = MT_SX * MT_SY;      // tile extents and field stride (elements)
+
+__device__ __forceinline__ void cp_async_elem(double* dst_smem, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(float* dst_smem, const float* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
+}
 
 // columns of tensor memory a block allocates: 8 warps share 4 lane quadrants, 3 kept values per evolved field
 template <typename R>
@@ -46,8 +71,11 @@ struct MarchTmem {
   }
 };
 
-template <typename R, bool VISC, int MODE>
-__global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> a, const int chunk) {
+#ifndef CLV_MARCH_MINB32
+#define CLV_MARCH_MINB32 3      // fp32 blocks per SM: 3 (<= 85 registers) measured 6.28 ms per step against 6.8 with 2
+#endif
+template <typename R, bool VISC, int MODE, bool TILE>
+__global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) stage_march_kernel(const StageArgs<R> a, const int chunk) {
   static_assert(MODE == 1 || MODE == 2, "the bootstrap (MODE 0) runs in the per-cell kernel");
   constexpr bool USE_PI = VISC;
   constexpr int NF = VISC ? 14 : 4;
@@ -62,6 +90,9 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
 
   __shared__ R sS[USE_PI ? 10 * 256 : 1];
   __shared__ unsigned s_tmem;
+  extern __shared__ __align__(16) unsigned char tile_raw[];      // TILE: R tile[NF + 5][12][36]
+  R* const tile = reinterpret_cast<R*>(tile_raw);
+  constexpr int NFT = NF + X_COUNT;
   using Priv = MarchTmem<R>;
   if (row == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)),
@@ -84,6 +115,32 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
     offy[p] = (int)(bmap(jc + p - 2, a.ny, a.bc[1]) * a.sy + xoff(ic, a.blk));
   }
   const long long cg0 = (long long)jc * a.gp + ic;
+  // tile fill: this thread copies the points tid and tid + 256 of the 36 x 12 halo'd tile, all fields (boundary rule a11
+  // applied to the source index, so the tile needs no special cases)
+  int tsrc[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const int pos = min(tid + 256 * s, MT_FST - 1);
+    const int r = pos / MT_SX, cx = pos - r * MT_SX;
+    tsrc[s] = (int)(bmap(blockIdx.y * 8 - 2 + r, a.ny, a.bc[1]) * a.sy +
+                    xoff(bmap(blockIdx.x * 32 - 2 + cx, a.nx, a.bc[0]), a.blk));
+  }
+  auto fill_tile = [&](int kk) {
+    const R* __restrict__ src = in + (long long)kk * a.sz;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      if (s == 0 || tid + 256 < MT_FST) {
+        const R* __restrict__ g0 = src + tsrc[s];
+        R* d0 = tile + (tid + 256 * s);
+#pragma unroll
+        for (int m = 0; m < NFT; ++m) cp_async_elem(d0 + m * MT_FST, g0 + m * FS);
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  constexpr bool ETILE = TILE && (CLV_MARCH_ETA_TILE != 0);
+  if (TILE) fill_tile(ETILE ? bmap(kc0 - 2, a.nz, a.bc[2]) : kc0);
+  const R* const town = tile + (row + 2) * MT_SX + (lane + 2);      // own point inside a field plane of the tile
 
   const R tf = a.milne ? a.tau : R(1);
   const R th2 = R(2) * a.theta;
@@ -93,7 +150,11 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
   for (int p = kc0; p <= kc1 + 1; ++p) {
     const int k = p - 2;
     const bool centre = p >= kc0 + 2;                      // block-uniform
-    if (CLV_MARCH_SYNC) __syncthreads();
+    if (CLV_MARCH_SYNC && !TILE) __syncthreads();
+    if (ETILE) {
+      asm volatile("cp.async.wait_all;" ::: "memory");
+      __syncthreads();                                     // tile(p-2) complete and visible
+    }
     const R* __restrict__ q2 = in + (long long)bmap(p - 2, a.nz, a.bc[2]) * a.sz + col;    // plane p-2 (= k)
     const R* __restrict__ q1 = in + (long long)bmap(p - 1, a.nz, a.bc[2]) * a.sz + col;
     const R* __restrict__ q0 = in + (long long)bmap(p, a.nz, a.bc[2]) * a.sz + col;
@@ -106,6 +167,23 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
       }
     }
 
+    if (CLV_MARCH_PF_TAIL && centre && (lane & (sizeof(R) == 8 ? 15 : 31)) == 0) {
+      const long long cpf = (long long)k * a.sz + col;
+      if (MODE == 2) {
+#pragma unroll
+        for (int m = 0; m < NF; ++m) prefetch_l1(a.sn + cpf + m * FS);
+        prefetch_l1(a.sn + cpf + OX + X_G * FS); prefetch_l1(a.sn + cpf + OX + X_P * FS);
+        if (USE_PI) prefetch_l1(a.gstar + (long long)k * a.ny * a.gp + cg0);
+      } else if (USE_PI) {
+#pragma unroll
+        for (int m = 0; m < 3; ++m) prefetch_l1(a.uprev + cpf + m * FS);
+      }
+      if (USE_PI) {
+        const R* __restrict__ zmp = in + (long long)bmap(k - 1, a.nz, a.bc[2]) * a.sz + col;
+        prefetch_l1(zmp + FS); prefetch_l1(zmp + 2 * FS); prefetch_l1(zmp + 3 * FS); prefetch_l1(zmp + OX + X_G * FS);
+      }
+    }
+
     R S[14];
 #pragma unroll
     for (int m = 0; m < 14; ++m) S[m] = R(0);
@@ -113,30 +191,32 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
     // ---- eta_s pipeline step: slope of cell p-1, face p-3/2, flux difference of cell p-2 ---------------------------
     {
       const R* __restrict__ pp[3] = {q2, q1, q0};
+      // field m of plane p-2+t at the own column (t is a constant after unrolling)
+#define ETA_LD(t, m) ((ETILE && (t) == 0) ? town[(m) * MT_FST] : pp[t][(m) * FS])
       R g[3], ua[3];
 #pragma unroll
-      for (int t = 0; t < 3; ++t) { g[t] = pp[t][OX + X_G * FS]; ua[t] = pp[t][3 * FS]; }
-      const R c2 = q2[OX + X_CN * FS];
+      for (int t = 0; t < 3; ++t) { g[t] = ETA_LD(t, NF + X_G); ua[t] = ETA_LD(t, 3); }
+      const R c2 = ETA_LD(0, NF + X_CN);
       const R cface = max_(c2, q1[OX + X_CN * FS]);
       cfl2 = c2 * a.h * a.scale[2];
       {
         R wq[3], wa[3], Pp[3];
 #pragma unroll
         for (int t = 0; t < 3; ++t) {
-          Pp[t] = pp[t][OX + X_P * FS];
-          const R w = pp[t][0] + Pp[t];
+          Pp[t] = ETA_LD(t, NF + X_P);
+          const R w = ETA_LD(t, 0) + Pp[t];
           wq[t] = w * g[t]; wa[t] = w * ua[t];
         }
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
           R q[3], f[3];
-          const int o_t = (F_PI + mu) * FS, o_a = (F_PI + c_pidx[3][mu]) * FS;
+          const int o_t = F_PI + mu, o_a = F_PI + c_pidx[3][mu];
 #pragma unroll
           for (int t = 0; t < 3; ++t) {
-            const R umu = mu == 0 ? g[t] : pp[t][mu * FS];
+            const R umu = mu == 0 ? g[t] : ETA_LD(t, mu);
             R tq = wq[t] * umu - (mu == 0 ? Pp[t] : R(0));
             R tfl = wa[t] * umu + (mu == 3 ? Pp[t] : R(0));
-            if (USE_PI) { tq += pp[t][o_t]; tfl += pp[t][o_a]; }
+            if (USE_PI) { tq += ETA_LD(t, o_t); tfl += ETA_LD(t, o_a); }
             q[t] = tq; f[t] = tfl;
           }
           R QLk, FLk, Hk, QL1, QR1, FL1, FR1;
@@ -159,7 +239,7 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
           R qa[3], fa_[3], qb[3], fb[3];
 #pragma unroll
           for (int s = 0; s < 3; ++s) {
-            const R va = pp[s][fa * FS], vb = pp[s][(fa + 1) * FS];
+            const R va = ETA_LD(s, fa), vb = ETA_LD(s, fa + 1);
             qa[s] = g[s] * va; fa_[s] = ua[s] * va;
             qb[s] = g[s] * vb; fb[s] = ua[s] * vb;
           }
@@ -178,14 +258,30 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
         }
       }
       tm_wait_st();
+#undef ETA_LD
     }
-    if (!centre) continue;
+    if (!centre) {
+      if (ETILE) { __syncthreads(); fill_tile(bmap(p - 1, a.nz, a.bc[2])); }
+      continue;
+    }
 
     // ---- x and y flux differences of cell k (five-point stars inside plane k) ---------------------------------------
     const R* __restrict__ plane = in + (long long)bmap(k, a.nz, a.bc[2]) * a.sz;
-    const R* __restrict__ pc = plane + col;
     R cfl0, cfl1;
-    {
+    if (TILE) {
+      if (!ETILE) {
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncthreads();                                   // tile(k) complete and visible
+      }
+      constexpr int OXT = NF * MT_FST;
+      const R* __restrict__ pp[5];
+#pragma unroll
+      for (int t = 0; t < 5; ++t) pp[t] = town + (t - 2);
+      axis_flux<R, USE_PI, 0, false, OXT, MT_FST>(a, pp, th2, tf, S, &sS[tid], cfl0);
+#pragma unroll
+      for (int t = 0; t < 5; ++t) pp[t] = town + (t - 2) * MT_SX;
+      axis_flux<R, USE_PI, 1, false, OXT, MT_FST>(a, pp, th2, tf, S, &sS[tid], cfl1);
+    } else {
       const R* __restrict__ pp[5];
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = plane + offx[t];
@@ -201,29 +297,59 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
 
     // ---- cell-centre state, velocity gradients ------------------------------------------------------------------------
     Cell<R> cc, cn_;
-    cc.e = pc[0];
-    cc.u[1] = pc[sf]; cc.u[2] = pc[2 * sf]; cc.u[3] = pc[3 * sf];
-    cc.u[0] = pc[OX + X_G * FS];
-    cc.P = pc[OX + X_P * FS];
-#pragma unroll
-    for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
     R grad[4][4];
 #pragma unroll
     for (int m = 0; m < 4; ++m)
 #pragma unroll
       for (int n = 0; n < 4; ++n) grad[m][n] = R(0);
-    if (USE_PI) {
-      const R* __restrict__ zm = in + (long long)bmap(k - 1, a.nz, a.bc[2]) * a.sz + col;
+    const R sc_x = R(0.5) * a.scale[0], sc_y = R(0.5) * a.scale[1], sc_n = R(0.5) * a.scale[2];
+    if (TILE) {
+      constexpr int OXT = NF * MT_FST;
+      cc.e = town[0];
+      cc.u[1] = town[MT_FST]; cc.u[2] = town[2 * MT_FST]; cc.u[3] = town[3 * MT_FST];
+      cc.u[0] = town[OXT + X_G * MT_FST];
+      cc.P = town[OXT + X_P * MT_FST];
 #pragma unroll
-      for (int ax = 0; ax < 3; ++ax) {
-        const R* __restrict__ qm = ax == 0 ? plane + offx[1] : (ax == 1 ? plane + offy[1] : zm);
-        const R* __restrict__ qp = ax == 0 ? plane + offx[3] : (ax == 1 ? plane + offy[3] : q1);
-        const R sc = R(0.5) * a.scale[ax];
-        grad[ax + 1][0] = (qp[OX + X_G * FS] - qm[OX + X_G * FS]) * sc;
-        grad[ax + 1][1] = (qp[sf] - qm[sf]) * sc;
-        grad[ax + 1][2] = (qp[2 * sf] - qm[2 * sf]) * sc;
-        grad[ax + 1][3] = (qp[3 * sf] - qm[3 * sf]) * sc;
+      for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? town[(F_PI + m) * MT_FST] : R(0);
+      if (USE_PI) {
+        grad[1][0] = (town[OXT + X_G * MT_FST + 1] - town[OXT + X_G * MT_FST - 1]) * sc_x;
+        grad[2][0] = (town[OXT + X_G * MT_FST + MT_SX] - town[OXT + X_G * MT_FST - MT_SX]) * sc_y;
+#pragma unroll
+        for (int n = 1; n < 4; ++n) {
+          grad[1][n] = (town[n * MT_FST + 1] - town[n * MT_FST - 1]) * sc_x;
+          grad[2][n] = (town[n * MT_FST + MT_SX] - town[n * MT_FST - MT_SX]) * sc_y;
+        }
       }
+      __syncthreads();                                     // every warp is done with tile(k): refill it for plane k+1,
+      if (ETILE) { if (p + 1 <= kc1 + 1) fill_tile(bmap(p - 1, a.nz, a.bc[2])); }
+      else if (k + 1 < kc1) fill_tile(k + 1);              // behind the stage tail below and the next eta_s step
+    } else {
+      const R* __restrict__ pc = plane + col;
+      cc.e = pc[0];
+      cc.u[1] = pc[sf]; cc.u[2] = pc[2 * sf]; cc.u[3] = pc[3 * sf];
+      cc.u[0] = pc[OX + X_G * FS];
+      cc.P = pc[OX + X_P * FS];
+#pragma unroll
+      for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
+      if (USE_PI) {
+#pragma unroll
+        for (int ax = 0; ax < 2; ++ax) {
+          const R* __restrict__ qm = ax == 0 ? plane + offx[1] : plane + offy[1];
+          const R* __restrict__ qp = ax == 0 ? plane + offx[3] : plane + offy[3];
+          const R sc = ax == 0 ? sc_x : sc_y;
+          grad[ax + 1][0] = (qp[OX + X_G * FS] - qm[OX + X_G * FS]) * sc;
+          grad[ax + 1][1] = (qp[sf] - qm[sf]) * sc;
+          grad[ax + 1][2] = (qp[2 * sf] - qm[2 * sf]) * sc;
+          grad[ax + 1][3] = (qp[3 * sf] - qm[3 * sf]) * sc;
+        }
+      }
+    }
+    if (USE_PI) {      // eta_s row: planes k-1 and k+1 of the own column
+      const R* __restrict__ zm = in + (long long)bmap(k - 1, a.nz, a.bc[2]) * a.sz + col;
+      grad[3][0] = (q1[OX + X_G * FS] - zm[OX + X_G * FS]) * sc_n;
+      grad[3][1] = (q1[sf] - zm[sf]) * sc_n;
+      grad[3][2] = (q1[2 * sf] - zm[2 * sf]) * sc_n;
+      grad[3][3] = (q1[3 * sf] - zm[3 * sf]) * sc_n;
     }
     const long long c = (long long)k * a.sz + col;
     const long long cg = (long long)k * a.ny * a.gp + cg0;
@@ -299,10 +425,10 @@ __global__ void __launch_bounds__(256, 2) stage_march_kernel(const StageArgs<R> 
   }
 }
 
-// planes per chunk: whole waves of the 2-blocks-per-SM residency, against the two pipeline warm-up planes of a chunk
-inline int march_chunk(int nx, int ny, int nz, int nsm) {
+// planes per chunk: whole waves of the resident blocks, against the two pipeline warm-up planes of a chunk
+inline int march_chunk(int nx, int ny, int nz, int nsm, int blocks_per_sm) {
   const long long tiles = (long long)((nx + 31) / 32) * ((ny + 7) / 8);
-  const long long slots = 2ll * nsm;
+  const long long slots = (long long)blocks_per_sm * nsm;
   double best = -1.0;
   int best_chunk = nz;
   for (int nchunk = 1; nchunk <= nz; ++nchunk) {
@@ -316,10 +442,21 @@ inline int march_chunk(int nx, int ny, int nz, int nsm) {
 }
 
 template <typename R, bool VISC, int MODE>
-void launch_stage_march(const StageArgs<R>& a, int chunk, cudaStream_t stream) {
+cudaError_t launch_stage_march(const StageArgs<R>& a, int chunk, cudaStream_t stream) {
+  constexpr bool TILE = CLV_MARCH_TILE != 0;
+  constexpr int NFT = (VISC ? 14 : 4) + X_COUNT;
+  const size_t smem = TILE ? (size_t)NFT * MT_FST * sizeof(R) : 0;
+  static bool configured = false;
+  if (TILE && !configured) {
+    cudaError_t e = cudaFuncSetAttribute(stage_march_kernel<R, VISC, MODE, TILE>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
   dim3 block(32, 8, 1);
   dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, (a.nz + chunk - 1) / chunk);
-  stage_march_kernel<R, VISC, MODE><<<grid, block, 0, stream>>>(a, chunk);
+  stage_march_kernel<R, VISC, MODE, TILE><<<grid, block, smem, stream>>>(a, chunk);
+  return cudaGetLastError();
 }
 
 }  // namespace clv

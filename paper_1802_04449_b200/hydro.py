@@ -33,7 +33,7 @@ class hydro_opts(Structure):
     _fields_ = [("precision", c_int), ("minmod_theta", c_double), ("e_floor", c_double),
                 ("pi_limit_xi", c_double), ("v_max", c_double), ("root_iters", c_int), ("kernel", c_int),
                 ("stream", c_void_p), ("workspace", c_void_p), ("workspace_bytes", c_size_t),
-                ("lambda1_hat", c_double), ("tau_pi_coeff", c_double)]
+                ("lambda1_hat", c_double), ("tau_pi_coeff", c_double), ("strict_eq53", c_int)]
 
 
 class hydro_diag_t(Structure):
@@ -122,7 +122,7 @@ class Hydro:
 
     def __init__(self, nx, ny, nz, dx, dy, deta, dtau, tau0, eos, eta_over_s, bc=(0, 0, 0), geometry=0,
                  precision=64, minmod_theta=1.1, e_floor=1e-7, pi_limit_xi=1.0, v_max=0.0, root_iters=0,
-                 kernel=0, device="cuda:0", stream=None, lambda1_hat=0.0, tau_pi_coeff=0.0):
+                 kernel=0, device="cuda:0", stream=None, lambda1_hat=0.0, tau_pi_coeff=0.0, strict_eq53=0):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -157,6 +157,7 @@ class Hydro:
             pi_limit_xi, v_max
         o.root_iters, o.kernel = root_iters, kernel
         o.lambda1_hat, o.tau_pi_coeff = lambda1_hat, tau_pi_coeff
+        o.strict_eq53 = int(strict_eq53)
         o.stream = c_void_p(self.stream.cuda_stream)
         o.workspace, o.workspace_bytes = c_void_p(aligned), nbytes
         with torch.cuda.device(self.device):
