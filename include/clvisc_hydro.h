@@ -71,7 +71,8 @@ typedef struct {
  * floor on e (A8); pi_limit_xi <= 0 switches the pi limiter off (A14); v_max: clamp of |M|/M0 (A7),
  * <= 0 selects the default 0.999 (gamma <= 22.4; A7 gives the evidence); root_iters: fixed Newton iteration
  * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
- * stream); workspace: DEVICE memory of at least hydro_workspace_bytes(), 256-byte aligned.
+ * stream); workspace: DEVICE memory of the current device, at least hydro_workspace_bytes(), 256-byte aligned (a host
+ * pointer or memory of another GPU is refused with HYDRO_EINVAL).
  * kernel: 0 = default (the fastest one as measured on B200: 4 in both precisions);
  * 4 = marching per-cell kernel (hydro_stage_march.cuh): kernel 2's store and x / y flux code, but a block walks along
  * eta_s and forms every eta_s slope and face once, with the per-column pipeline state in tensor memory;

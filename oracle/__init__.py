@@ -40,7 +40,8 @@ def _bind(path):
     lib.oracle_destroy.argtypes = [ctypes.c_void_p]
     for name, nptr in [("oracle_load", 2), ("oracle_set_history", 1), ("oracle_read", 3),
                        ("oracle_read_T", 1), ("oracle_read_history", 1), ("oracle_diag", 1),
-                       ("oracle_set_state", 3)]:
+                       ("oracle_set_state", 3), ("oracle_load_ext", 4), ("oracle_read_ext", 2),
+                       ("oracle_set_ext", 2)]:
         f = getattr(lib, name)
         f.restype = ctypes.c_int
         f.argtypes = [ctypes.c_void_p] + [dp] * nptr
@@ -168,7 +169,26 @@ class Oracle:
         acted = self._lib.oracle_limit_pi(self._h, float(e), _p(p))
         return p, bool(acted)
 
-    OPT_HEUN_PRINTED, OPT_LAMBDA1_HAT, OPT_C_TAU = 0, 1, 2
+    OPT_HEUN_PRINTED, OPT_LAMBDA1_HAT, OPT_C_TAU, OPT_EXT, OPT_ZETA_S = 0, 1, 2, 3, 4
+
+    # -- bulk pressure Pi and net-baryon density n (after set_option(OPT_EXT, 1)) -------------
+    def load_ext(self, T, pi=None, Pi=None, nb=None):
+        T = np.ascontiguousarray(T, dtype=np.float64).reshape(4, -1)
+        pi = None if pi is None else np.ascontiguousarray(pi, dtype=np.float64).reshape(10, -1)
+        Pi = None if Pi is None else np.ascontiguousarray(Pi, dtype=np.float64).reshape(-1)
+        nb = None if nb is None else np.ascontiguousarray(nb, dtype=np.float64).reshape(-1)
+        return self._lib.oracle_load_ext(self._h, _p(T), _p(pi), _p(Pi), _p(nb))
+
+    def set_ext(self, Pi=None, nb=None):
+        Pi = None if Pi is None else np.ascontiguousarray(Pi, dtype=np.float64).reshape(-1)
+        nb = None if nb is None else np.ascontiguousarray(nb, dtype=np.float64).reshape(-1)
+        if self._lib.oracle_set_ext(self._h, _p(Pi), _p(nb)):
+            raise ValueError("oracle_set_ext: the extension is off (set_option(OPT_EXT, 1) on a viscous run)")
+
+    def read_ext(self):
+        Pi, nb = np.empty(self.N), np.empty(self.N)
+        self._lib.oracle_read_ext(self._h, _p(Pi), _p(nb))
+        return Pi.reshape(self.shape), nb.reshape(self.shape)
 
     def set_option(self, key, value):
         if self._lib.oracle_set_option(self._h, int(key), float(value)):

@@ -102,6 +102,22 @@ struct Oracle {
   // needed by the paper's closed-form Gubser test (L = 2, eta_v/s = 0.2, lambda1_hat = -10 and
   // tau_pi from eta_hat lambda1_hat^2 = 3 tau_pi_hat, i.e. c_tau = 4 lambda1_hat^2 / 9).
   double lambda1_hat = 0.0, c_tau = 5.0;
+  // SURVEY 8(f)-3 (PAPER.md:46-56 Eq.1-3; :153-171 Eq.28, 30, 32, 34; :614 "2 components in N and Pi": the 16-word cell):
+  // bulk pressure Pi and net-baryon density n (local rest frame), evolved when ext = 1 (viscous runs only).
+  //   A28  T_f^{mu nu} = (e + P + Pi) u~^mu u~^nu - (P + Pi) g~^{mu nu} + pi~^{mu nu}                    (Eq.1, :50)
+  //   A29  S_Pi,tot = S_KT - (Pi + zeta theta~)/tau_Pi - Pi theta~/3 - u~^tau Pi / tau: Eq.3 (:56), the defining equation,
+  //        written as a balance law, d_mu(u^mu Pi) = D Pi + Pi theta with D Pi = -(Pi + zeta theta)/tau_Pi - 4/3 Pi theta;
+  //        the printed Eq.34 has +zeta theta~ (against Eq.3 and against the Navier-Stokes limit Pi = -zeta theta) and lacks
+  //        the Milne term u~^tau Pi / tau that its shear twin Eq.33 carries (sign as A1)
+  //   A30  zeta = (zeta/s) s with s = (e+P)/T and a constant zeta/s; tau_Pi = tau_pi (the paper leaves both open, :72)
+  //   A31  N~^mu = tau n u~^mu (Eq.21, :128), S_N = 0 (Eq.32): Q_N = tau n u~^tau, F_a = tau n u~^a; n = Q_N/(tau u~^tau)
+  //        after the root-find; the EoS does not depend on n (P(e) tables, :253-259)
+  //   A32  the root-find carries Pi: e = M0 - M^2/(M0 + P(e) + Pi), v = M/(M0 + P + Pi); afterwards |Pi| <= xi P(e)
+  //        (same xi as the pi limiter) -- a convention in the spirit of A14, "parity unpinned" beyond its invariant
+  int ext = 0;
+  double zeta_s = 0.0;
+  std::vector<double> Pi, nB;
+  long n_bulk_limit = 0;
   int step = 0;
   bool loaded = false;
   size_t N;
@@ -131,6 +147,8 @@ struct State {
   const double* e;
   const double* u[3];
   const double* pi[10];  // all null => ideal (pi == 0)
+  const double* Pi = nullptr;   // 8(f)-3: bulk pressure (null => 0) and net-baryon density (null => not evolved)
+  const double* nB = nullptr;
 };
 
 // Full frame tensor T_f^{mu nu} at one cell (Eq.1 :50 in tilde components, Eq.18-23).
@@ -140,6 +158,7 @@ void frame_tensor(const Oracle& o, const State& s, size_t c, bool use_pi, double
   ut[0] = std::sqrt(1.0 + ux * ux + uy * uy + un * un);
   ut[1] = ux; ut[2] = uy; ut[3] = un;
   double e = s.e[c];
+  if (s.Pi) P += s.Pi[c];       // A28: the bulk pressure adds to the equilibrium pressure in T_f
   for (int m = 0; m < 4; ++m)
     for (int n = 0; n < 4; ++n) {
       double t = (e + P) * ut[m] * ut[n];
@@ -159,8 +178,8 @@ double signal_speed(double va, double v2, double cs2) {
 // Workspace of per-point quantities for one RHS evaluation (steps 1-2 of SURVEY 8c).
 struct PointTables {
   std::vector<double> P, cs2, T;
-  std::vector<double> Q[14];
-  std::vector<double> F[14];
+  std::vector<double> Q[16];
+  std::vector<double> F[16];
   std::vector<double> c;
 };
 
@@ -179,10 +198,12 @@ double kt_face(double theta, const std::vector<double>& Q, const std::vector<dou
 // RHS operator R(e, u~, d_tau u~, pi~; tau) -> S_T,tot[4], S_pi,tot[10]  (Eq.45-48).
 // dtu[4]: arrays of d_tau u~^mu.  use_pi=false: ideal fluid (pi terms skipped, A15).
 // cfl_out (optional, 3 values): max over cells of c_a*h/Delta_a.
+// SX (optional, with s.Pi / s.nB set): S_Pi,tot and S_N,tot (8(f)-3).
 void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>* dtu, double tau,
-         std::vector<double>* ST, std::vector<double>* SP, double* cfl_out) {
+         std::vector<double>* ST, std::vector<double>* SP, double* cfl_out, std::vector<double>* SX = nullptr) {
   const size_t N = o.N;
-  const int nf = use_pi ? 14 : 4;
+  const bool ext = use_pi && s.Pi && s.nB && SX;
+  const int nf = use_pi ? (ext ? 16 : 14) : 4;
   const bool milne = (o.geometry == 0);
   const double tf = milne ? tau : 1.0;  // Q_T = tau*T_f^{tau mu}; Cartesian: factor 1
   PointTables pt;
@@ -190,6 +211,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
   for (int m = 0; m < nf; ++m) { pt.Q[m].resize(N); pt.F[m].resize(N); }
   for (int m = 0; m < 4; ++m) ST[m].assign(N, 0.0);
   if (use_pi) for (int m = 0; m < 10; ++m) SP[m].assign(N, 0.0);
+  if (ext) { SX[0].assign(N, 0.0); SX[1].assign(N, 0.0); }
 
   // step 1-2: EoS and conserved variables at every cell
 #pragma omp parallel for
@@ -199,6 +221,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
     frame_tensor(o, s, c, use_pi, pt.P[c], Tf, ut);
     for (int m = 0; m < 4; ++m) pt.Q[m][c] = tf * Tf[0][m];
     if (use_pi) for (int m = 0; m < 10; ++m) pt.Q[4 + m][c] = ut[0] * s.pi[m][c];
+    if (ext) { pt.Q[14][c] = ut[0] * s.Pi[c]; pt.Q[15][c] = tf * s.nB[c] * ut[0]; }      // Eq.30; Eq.28 with A31
   }
 
   // steps 2-5: per axis, fluxes F_a, signal speed c_a, KT divergence (Eq.40); order x, y, eta (A22)
@@ -211,6 +234,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
       frame_tensor(o, s, c, use_pi, pt.P[c], Tf, ut);
       for (int m = 0; m < 4; ++m) pt.F[m][c] = tf * Tf[a + 1][m];
       if (use_pi) for (int m = 0; m < 10; ++m) pt.F[4 + m][c] = ut[a + 1] * s.pi[m][c];
+      if (ext) { pt.F[14][c] = ut[a + 1] * s.Pi[c]; pt.F[15][c] = tf * s.nB[c] * ut[a + 1]; }
       double g = ut[0];
       double v2 = (ut[1] * ut[1] + ut[2] * ut[2] + ut[3] * ut[3]) / (g * g);
       pt.c[c] = signal_speed(ut[a + 1] / g, v2, pt.cs2[c]);
@@ -228,7 +252,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
         double Hr = kt_face(o.theta, pt.Q[m], pt.F[m], cr, m1, c, p1, p2);
         double Hl = kt_face(o.theta, pt.Q[m], pt.F[m], cl, m2, m1, c, p1);
         double div = -(Hr - Hl) * scale;
-        if (m < 4) ST[m][c] += div; else SP[m - 4][c] += div;
+        if (m < 4) ST[m][c] += div; else if (m < 14) SP[m - 4][c] += div; else SX[m - 14][c] += div;
       }
     }
   }
@@ -270,6 +294,12 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
     double e = s.e[c], P = pt.P[c], T = pt.T[c];
     double inv_taupi = T / (o.c_tau * o.eta_s * HBARC);     // tau_pi = 5 eta_v/(T s)
     double etav_over_taupi = (e + P) / o.c_tau;             // eta_v/tau_pi = (e+P)/5
+    if (ext) {   // A29, A30: tau_Pi = tau_pi, zeta/tau_Pi = (zeta/s)/(eta_v/s) (e+P)/c_tau; S_N = 0 (Eq.32)
+      double Pb = s.Pi[c];
+      double src = -Pb * inv_taupi - (o.zeta_s / o.eta_s) * etav_over_taupi * theta_exp - Pb * theta_exp / 3.0;
+      if (milne) src -= Pb * ut[0] / tau;
+      SX[0][c] += src;
+    }
     auto pic = [&](int m, int n) { return s.pi[PIDX[m][n]][c]; };
     // lambda_1 term (Eq.33): -(lambda_1/tau_pi) pi~^{<mu}_lambda pi~^{nu>lambda}, with the projector
     // of Eq.5 written out: X^{ab} = pi~^{a l} g~_{l k} pi~^{k b};  X^{<mn>} = Delta^{mn}_{ab} X^{ab},
@@ -321,7 +351,9 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
 }
 
 // Root-find T_id^{tau mu} -> e, u~^i  (Eq.51/54; A7, A8).  M[4] = (M0, Mx, My, Meta).
-void rootfind(Oracle& o, const double M[4], double* e_out, double u_out[3], long* nfloor, long* nclamp) {
+// Pib: bulk pressure carried through the root-find (A32; 0 without 8(f)-3).
+void rootfind(Oracle& o, const double M[4], double* e_out, double u_out[3], long* nfloor, long* nclamp,
+              double Pib = 0.0) {
   double M0 = M[0];
   if (!(M0 > o.e_floor)) {
     *e_out = o.e_floor; u_out[0] = u_out[1] = u_out[2] = 0.0; ++*nfloor;
@@ -340,6 +372,7 @@ void rootfind(Oracle& o, const double M[4], double* e_out, double u_out[3], long
   for (int it = 0; it < 200; ++it) {
     double P, cs2, T;
     eos_eval(o.eos, e, &P, &cs2, &T);
+    P += Pib;
     double g = M0 - Mabs * Mabs / (M0 + P) - e;
     if (std::fabs(g) <= 1e-15 * M0) break;
     if (g > 0) lo = e; else hi = e;
@@ -352,6 +385,7 @@ void rootfind(Oracle& o, const double M[4], double* e_out, double u_out[3], long
   if (e < o.e_floor) { e = o.e_floor; ++*nfloor; }
   double P, cs2, T;
   eos_eval(o.eos, e, &P, &cs2, &T);
+  P += Pib;
   double v[3], v2 = 0;
   for (int a = 0; a < 3; ++a) { v[a] = Mi[a] / (M0 + P); v2 += v[a] * v[a]; }
   double gam = 1.0 / std::sqrt(1.0 - v2);
@@ -369,6 +403,15 @@ void limit_pi(const Oracle& o, double e, double pi[10], long* nlimit) {
   double mag = std::sqrt(std::fabs(pp));
   double r = o.xi * std::sqrt(e * e + 3.0 * P * P) / std::max(mag, 1e-300);
   if (r < 1.0) { for (int m = 0; m < 10; ++m) pi[m] *= r; ++*nlimit; }
+}
+
+// Bulk limiter (A32): |Pi| <= xi P(e), so that P + Pi >= 0 for xi <= 1.
+void limit_bulk(const Oracle& o, double e, double* Pib, long* nlimit) {
+  if (!(o.xi > 0)) return;
+  double P, cs2, T;
+  eos_eval(o.eos, e, &P, &cs2, &T);
+  double lim = o.xi * P;
+  if (std::fabs(*Pib) > lim) { *Pib = std::copysign(lim, *Pib); ++*nlimit; }
 }
 
 State view(const std::vector<double>& e, const std::vector<double>* u, const std::vector<double>* pi,
@@ -432,29 +475,42 @@ void step_once(Oracle& o) {
     dtu[0][c] = (gstar[c] - std::sqrt(g2)) / h;          // A10
     for (int a = 0; a < 3; ++a) dtu[a + 1][c] = (us[a] - o.u[a][c]) / h;
   }
+  const bool ext = visc && o.ext;
   State sn = view(o.e, o.u, o.pi, visc);
-  std::vector<double> ST[4], SP[10];
-  rhs(o, sn, visc, dtu, tau_n, ST, SP, o.cfl);
+  if (ext) { sn.Pi = o.Pi.data(); sn.nB = o.nB.data(); }
+  std::vector<double> ST[4], SP[10], SX[2];
+  rhs(o, sn, visc, dtu, tau_n, ST, SP, o.cfl, ext ? SX : nullptr);
 
   std::vector<double> e1(N), u1[3], pi1[10], QTn[4];
   for (int a = 0; a < 3; ++a) u1[a].resize(N);
   for (int m = 0; m < 10; ++m) pi1[m].assign(N, 0.0);
   for (int m = 0; m < 4; ++m) QTn[m].resize(N);
-  long nfl = 0, ncl = 0, nli = 0;   // event counters of this step (summed over the flat cell loops)
-#pragma omp parallel for reduction(+ : nfl, ncl, nli)
+  std::vector<double> Pi1, nb1, QNn;   // 8(f)-3: Pi', n' and Q_N^n
+  if (ext) { Pi1.assign(N, 0.0); nb1.assign(N, 0.0); QNn.assign(N, 0.0); }
+  long nfl = 0, ncl = 0, nli = 0, nbl = 0;   // event counters of this step (summed over the flat cell loops)
+#pragma omp parallel for reduction(+ : nfl, ncl, nli, nbl)
   for (size_t c = 0; c < N; ++c) {
     double QT[4], pp[10] = {0}, M[4], uu[3];
     conserved_T(o, sn, c, visc, tf_n, QT);
     for (int m = 0; m < 4; ++m) QTn[m][c] = QT[m];
+    double gn = 1.0, Pb = 0.0;
     if (visc) {
-      double gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
+      gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
       for (int m = 0; m < 10; ++m) pp[m] = (gn * o.pi[m][c] + h * SP[m][c]) / gstar[c];   // Eq.49
     }
+    if (ext) Pb = (gn * o.Pi[c] + h * SX[0][c]) / gstar[c];                                // Eq.48 like Eq.49
     for (int m = 0; m < 4; ++m) M[m] = (QT[m] + h * ST[m][c]) / tf_1 - pp[m];              // Eq.50-51
-    rootfind(o, M, &e1[c], uu, &nfl, &ncl);
+    rootfind(o, M, &e1[c], uu, &nfl, &ncl, Pb);
     if (visc) limit_pi(o, e1[c], pp, &nli);
     for (int a = 0; a < 3; ++a) u1[a][c] = uu[a];
     for (int m = 0; m < 10; ++m) pi1[m][c] = pp[m];
+    if (ext) {
+      limit_bulk(o, e1[c], &Pb, &nbl);
+      Pi1[c] = Pb;
+      QNn[c] = tf_n * o.nB[c] * gn;                                                        // Eq.46, A31
+      double g1 = std::sqrt(1.0 + uu[0] * uu[0] + uu[1] * uu[1] + uu[2] * uu[2]);
+      nb1[c] = (QNn[c] + h * SX[1][c]) / (tf_1 * g1);
+    }
   }
 
   // ---- stage 2 at tau_{n+1} ---------------------------------------------------------------
@@ -466,8 +522,9 @@ void step_once(Oracle& o) {
     for (int a = 0; a < 3; ++a) dtu[a + 1][c] = (u1[a][c] - o.u[a][c]) / h;   // (u' - u^n)/h, A10
   }
   State s1 = view(e1, u1, pi1, visc);
-  std::vector<double> ST1[4], SP1[10];
-  rhs(o, s1, visc, dtu, tau_1, ST1, SP1, nullptr);
+  if (ext) { s1.Pi = Pi1.data(); s1.nB = nb1.data(); }
+  std::vector<double> ST1[4], SP1[10], SX1[2];
+  rhs(o, s1, visc, dtu, tau_1, ST1, SP1, nullptr, ext ? SX1 : nullptr);
 
   // Heun in Shu-Osher form (A26, default): Q^{n+1} = 1/2 [Q^n + Q(state') + h S_tot(state')], where
   // Q(state') is rebuilt from the stored stage-1 state (after floor / clamp / limiter).
@@ -493,24 +550,41 @@ void step_once(Oracle& o) {
       rhs(o, s1b, true, dtu, tau_1, ST1, SPdummy, nullptr);
     }
   }
-#pragma omp parallel for reduction(+ : nfl, ncl, nli)
+#pragma omp parallel for reduction(+ : nfl, ncl, nli, nbl)
   for (size_t c = 0; c < N; ++c) {
     double QT1[4], M[4], pp[10], en, uu[3];
     conserved_T(o, s1, c, visc, tf_1, QT1);
     for (int m = 0; m < 10; ++m) pp[m] = pinew[m][c];
+    double Pb = 0.0, QNnew = 0.0;
+    if (ext) {   // Heun for Pi and Q_N in the same bookkeeping as pi and Q_T (A26)
+      double gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
+      double g1 = std::sqrt(1.0 + u1[0][c] * u1[0][c] + u1[1][c] * u1[1][c] + u1[2][c] * u1[2][c]);
+      if (o.heun_printed) {
+        Pb = (gn * o.Pi[c] + 0.5 * h * (SX[0][c] + SX1[0][c])) / g1;
+        QNnew = QNn[c] + 0.5 * h * (SX[1][c] + SX1[1][c]);
+      } else {
+        Pb = 0.5 * (gn * o.Pi[c] + gstar[c] * Pi1[c] + h * SX1[0][c]) / g1;
+        QNnew = 0.5 * (QNn[c] + tf_1 * nb1[c] * g1 + h * SX1[1][c]);
+      }
+    }
     for (int m = 0; m < 4; ++m) {
       if (o.heun_printed)
         M[m] = (QTn[m][c] + 0.5 * h * (ST[m][c] + ST1[m][c])) / tf_1 - pp[m];                // Eq.53-54 as printed
       else
         M[m] = 0.5 * (QTn[m][c] + QT1[m] + h * ST1[m][c]) / tf_1 - pp[m];                    // Eq.53-54
     }
-    rootfind(o, M, &en, uu, &nfl, &ncl);
+    rootfind(o, M, &en, uu, &nfl, &ncl, Pb);
     if (visc) limit_pi(o, en, pp, &nli);
     for (int a = 0; a < 3; ++a) { o.uprev[a][c] = o.u[a][c]; o.u[a][c] = uu[a]; }
     o.e[c] = en;
     for (int m = 0; m < 10; ++m) o.pi[m][c] = pp[m];
+    if (ext) {
+      limit_bulk(o, en, &Pb, &nbl);
+      o.Pi[c] = Pb;
+      o.nB[c] = QNnew / (tf_1 * std::sqrt(1.0 + uu[0] * uu[0] + uu[1] * uu[1] + uu[2] * uu[2]));
+    }
   }
-  o.n_floor += nfl; o.n_clamp += ncl; o.n_limit += nli;
+  o.n_floor += nfl; o.n_clamp += ncl; o.n_limit += nli; o.n_bulk_limit += nbl;
   o.e_max_seen = *std::max_element(o.e.begin(), o.e.end());
   o.step += 1;
 }
@@ -547,17 +621,21 @@ void* oracle_create(int nx, int ny, int nz, double dx, double dy, double deta, c
 
 void oracle_destroy(void* h) { delete static_cast<Oracle*>(h); }
 
-// T: T_f^{tau mu} [4][N] (no extra factor tau); pi: pi~ [10][N] or NULL.
-int oracle_load(void* h, const double* T, const double* pi) {
+// T: T_f^{tau mu} [4][N] (no extra factor tau); pi: pi~ [10][N] or NULL.  8(f)-3 (ext = 1): Pi [N] and nb [N] (NULL = 0);
+// T is then the full tensor, including the bulk pressure (A28), and the root-find carries Pi (A32).
+int oracle_load_ext(void* h, const double* T, const double* pi, const double* Pi, const double* nb) {
   Oracle& o = *static_cast<Oracle*>(h);
   const size_t N = o.N;
+  const bool ext = o.ext && o.viscous();
+  if (ext) { o.Pi.assign(N, 0.0); o.nB.assign(N, 0.0); }
   long nfl = 0, ncl = 0;
 #pragma omp parallel for reduction(+ : nfl, ncl)
   for (size_t c = 0; c < N; ++c) {
     double M[4], uu[3];
     for (int m = 0; m < 10; ++m) o.pi[m][c] = (pi && o.viscous()) ? pi[m * N + c] : 0.0;
     for (int m = 0; m < 4; ++m) M[m] = T[m * N + c] - o.pi[m][c];
-    rootfind(o, M, &o.e[c], uu, &nfl, &ncl);
+    if (ext) { o.Pi[c] = Pi ? Pi[c] : 0.0; o.nB[c] = nb ? nb[c] : 0.0; }
+    rootfind(o, M, &o.e[c], uu, &nfl, &ncl, ext ? o.Pi[c] : 0.0);
     for (int a = 0; a < 3; ++a) o.u[a][c] = uu[a];
   }
   o.n_floor += nfl; o.n_clamp += ncl;
@@ -565,6 +643,19 @@ int oracle_load(void* h, const double* T, const double* pi) {
   bootstrap_history(o);
   o.e_max_seen = *std::max_element(o.e.begin(), o.e.end());
   o.loaded = true;
+  return 0;
+}
+
+int oracle_load(void* h, const double* T, const double* pi) { return oracle_load_ext(h, T, pi, nullptr, nullptr); }
+
+// 8(f)-3: bulk pressure Pi [N] and net-baryon density n [N] of the current state; either may be NULL.
+int oracle_read_ext(void* h, double* Pi, double* nb) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const bool ext = o.ext && o.viscous();
+  for (size_t c = 0; c < o.N; ++c) {
+    if (Pi) Pi[c] = ext ? o.Pi[c] : 0.0;
+    if (nb) nb[c] = ext ? o.nB[c] : 0.0;
+  }
   return 0;
 }
 
@@ -601,6 +692,7 @@ int oracle_read(void* h, double* e, double* u, double* pi) {
 int oracle_read_T(void* h, double* T) {
   Oracle& o = *static_cast<Oracle*>(h);
   State s = view(o.e, o.u, o.pi, o.viscous());
+  if (o.ext && o.viscous() && o.Pi.size() == o.N) s.Pi = o.Pi.data();      // 8(f)-3: the full tensor (A28)
   for (size_t c = 0; c < o.N; ++c) {
     double QT[4];
     conserved_T(o, s, c, o.viscous(), 1.0, QT);
@@ -649,7 +741,18 @@ int oracle_set_state(void* h, const double* e, const double* u, const double* pi
   for (int m = 0; m < 10; ++m)
     for (size_t c = 0; c < N; ++c) o.pi[m][c] = (pi && o.viscous()) ? pi[m * N + c] : 0.0;
   o.uprev[0] = o.u[0]; o.uprev[1] = o.u[1]; o.uprev[2] = o.u[2];
+  if (o.ext && o.viscous()) { o.Pi.assign(N, 0.0); o.nB.assign(N, 0.0); }
   o.step = 0; o.loaded = true;
+  return 0;
+}
+
+// 8(f)-3: set Pi [N] and n [N] of the current state directly (after oracle_set_state); NULL leaves a field as it is.
+int oracle_set_ext(void* h, const double* Pi, const double* nb) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (!(o.ext && o.viscous())) return -1;
+  if (o.Pi.size() != o.N) { o.Pi.assign(o.N, 0.0); o.nB.assign(o.N, 0.0); }
+  if (Pi) std::copy(Pi, Pi + o.N, o.Pi.begin());
+  if (nb) std::copy(nb, nb + o.N, o.nB.begin());
   return 0;
 }
 
@@ -667,12 +770,16 @@ int oracle_limit_pi(void* h, double e, double* pi10) {
 }
 
 // Options that are not part of oracle_create's argument list.  key 0: heun_printed (A26; 0 default, 1 = Eq.52-53
-// as printed); key 1: lambda1_hat; key 2: c_tau.  Returns 0, or -1 for an unknown key / bad value.
+// as printed); key 1: lambda1_hat; key 2: c_tau; keys 3, 4: SURVEY 8(f)-3.  Returns 0, or -1 for an
+// unknown key / bad value.
 int oracle_set_option(void* h, int key, double value) {
   Oracle& o = *static_cast<Oracle*>(h);
   if (key == 0) { o.heun_printed = value != 0.0 ? 1 : 0; return 0; }
   if (key == 1) { o.lambda1_hat = value; return 0; }
   if (key == 2) { if (!(value > 0.0)) return -1; o.c_tau = value; return 0; }
+  // key 3: evolve Pi and n (8(f)-3; viscous runs without strict_eq53 only); key 4: zeta/s >= 0 (A30)
+  if (key == 3) { if (value != 0.0 && (!o.viscous() || o.strict_eq53)) return -1; o.ext = value != 0.0 ? 1 : 0; return 0; }
+  if (key == 4) { if (!(value >= 0.0)) return -1; o.zeta_s = value; return 0; }
   return -1;
 }
 

@@ -732,6 +732,16 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
     return HYDRO_ENOMEM;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { (void)cudaGetLastError(); return HYDRO_ECUDA; }
+  {   // the workspace must be device memory of the CURRENT device (a host or wrong-GPU pointer would fault inside a kernel)
+    cudaPointerAttributes pa;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaPointerGetAttributes(&pa, opts->workspace) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return HYDRO_ECUDA;
+    }
+    if ((pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged) || (pa.type == cudaMemoryTypeDevice && pa.device != dev))
+      return HYDRO_EINVAL;
+  }
 
   hydro_ctx* c = new (std::nothrow) hydro_ctx();
   if (!c) return HYDRO_ENOMEM;

@@ -86,3 +86,23 @@ def test_product_never_imports_oracle():
         if f.endswith((".py", ".cpp")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_1802_04449_b200" not in txt and "libclvisc_hydro" not in txt, f
+
+
+@pytest.mark.gpu
+def test_create_refuses_a_host_workspace():
+    """hydro_create checks the workspace with cudaPointerGetAttributes: host memory is HYDRO_EINVAL, not a fault in a
+    kernel later."""
+    import numpy as np
+    from paper_1802_04449_b200 import hydro
+    lib = hydro.load_library()
+    g = hydro.make_grid(8, 8, 8, 0.1, 0.1, 0.1)
+    e = hydro.hydro_eos(); e.kind, e.n, e.e_min, e.e_max, e.c_sb = 0, 0, 0.0, 0.0, 15.6
+    o = hydro.hydro_opts()
+    o.precision, o.minmod_theta, o.e_floor, o.pi_limit_xi, o.v_max = 64, 1.1, 1e-7, 1.0, 0.0
+    nbytes = hydro.workspace_bytes(g, 64, 0.1)
+    host = np.zeros(nbytes + 256, dtype=np.uint8)
+    base = (host.ctypes.data + 255) // 256 * 256
+    o.workspace, o.workspace_bytes = c_void_p(base), nbytes
+    h = c_void_p()
+    assert lib.hydro_create(byref(h), byref(g), 0.01, 0.6, byref(e), 0.1, byref(o)) == -1
+    assert not h.value
