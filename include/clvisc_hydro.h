@@ -97,6 +97,15 @@ typedef struct {
    * evaluated with pi^{n+1} (the result of Eq.52) instead of pi': stage 2 becomes three launches (4 per RK2 step).
    * Kernels 2 and 4 only (HYDRO_EINVAL otherwise); ignored for eta_over_s = 0.  0 = standard Heun (default). */
   int strict_eq53;
+  /* SURVEY 8(f)-3 (PAPER.md:46-56 Eq.1-3; :153-171 Eq.28, 30, 32, 34; :614 the 16-word cell): bulk_baryon = 1 evolves the
+   * bulk pressure Pi and the net-baryon density n next to T^{tau mu} and pi^{mu nu} (readings A28-A32):
+   *   T_f^{mu nu} = (e + P + Pi) u u - (P + Pi) g + pi;   d_mu(u^mu Pi) = -(Pi + zeta theta)/tau_Pi - Pi theta/3 with
+   *   tau_Pi = tau_pi and zeta = zeta_over_s * s;   d~_mu(tau n u~^mu) = 0;   root-find with P + Pi;   |Pi| <= xi P.
+   * Viscous runs only, per-cell fused kernel (opts->kernel 0, 2 or 4; it runs kernel 2), not with strict_eq53; needs
+   * hydro_workspace_bytes_ext(); state loaded / read with hydro_load_ext / hydro_read_ext.  0 = off (the paper's setting,
+   * "bulk viscosity and net baryon density are set to 0 in the current version"). */
+  int bulk_baryon;
+  double zeta_over_s;
 } hydro_opts;
 
 /* Diagnostics (PAPER.md:640 for e_max).  cfl[a] = max over cells of
@@ -112,6 +121,9 @@ typedef struct {
 /* Bytes of device workspace a context for this grid/precision/viscosity needs (0 on bad input). */
 size_t hydro_workspace_bytes(const hydro_grid *grid, int precision, double eta_over_s);
 
+/* As hydro_workspace_bytes, for a context created with opts->bulk_baryon (16 evolved words per cell). */
+size_t hydro_workspace_bytes_ext(const hydro_grid *grid, int precision, double eta_over_s, int bulk_baryon);
+
 /* Create a context.  tau0: initial proper time (fm/c), dtau: fixed step h; eta_over_s = 0 selects
  * the ideal-fluid path (no pi array is touched, A15).  Errors: HYDRO_EINVAL (bad sizes, precision,
  * theta, table), HYDRO_ENOMEM (workspace too small or misaligned), HYDRO_ECUDA. */
@@ -122,6 +134,12 @@ int hydro_create(hydro_ctx **out, const hydro_grid *grid, double dtau, double ta
  * (= 0).  Root-finds the primitives (Eq.51), bootstraps u^{-1} with one ideal-fluid predictor
  * (A23), resets tau, step and counters.  mem: HYDRO_MEM_DEVICE / HYDRO_MEM_HOST. */
 int hydro_load(hydro_ctx *ctx, const void *T_tau_mu, const void *pi_mu_nu, int mem);
+
+/* SURVEY 8(f)-3, contexts created with opts->bulk_baryon: hydro_load with two more fields, Pi [nz][ny][nx] and the
+ * net-baryon density n [nz][ny][nx] (either may be NULL = 0).  T_tau_mu is the FULL tensor including the bulk pressure.
+ * hydro_read_ext returns Pi and n of the current state (either may be NULL).  HYDRO_ESTATE on other contexts. */
+int hydro_load_ext(hydro_ctx *ctx, const void *T_tau_mu, const void *pi_mu_nu, const void *Pi, const void *n_b, int mem);
+int hydro_read_ext(hydro_ctx *ctx, void *Pi, void *n_b, int mem);
 
 /* Overwrite / read the history u~^i at step n-1, [3][nz][ny][nx] (analytic tests, bitwise resume). */
 int hydro_set_history(hydro_ctx *ctx, const void *u_prev, int mem);

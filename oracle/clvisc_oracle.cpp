@@ -112,7 +112,8 @@ struct Oracle {
   //   A30  zeta = (zeta/s) s with s = (e+P)/T and a constant zeta/s; tau_Pi = tau_pi (the paper leaves both open, :72)
   //   A31  N~^mu = tau n u~^mu (Eq.21, :128), S_N = 0 (Eq.32): Q_N = tau n u~^tau, F_a = tau n u~^a; n = Q_N/(tau u~^tau)
   //        after the root-find; the EoS does not depend on n (P(e) tables, :253-259)
-  //   A32  the root-find carries Pi: e = M0 - M^2/(M0 + P(e) + Pi), v = M/(M0 + P + Pi); afterwards |Pi| <= xi P(e)
+  //   A32  the root-find carries Pi through the total pressure P_tot(e) = max(P(e) + Pi, 0) (continuous, non-decreasing:
+  //        the root stays unique and |v| <= v_max): e = M0 - M^2/(M0 + P_tot), v = M/(M0 + P_tot); afterwards |Pi| <= xi P(e)
   //        (same xi as the pi limiter) -- a convention in the spirit of A14, "parity unpinned" beyond its invariant
   int ext = 0;
   double zeta_s = 0.0;
@@ -372,7 +373,7 @@ void rootfind(Oracle& o, const double M[4], double* e_out, double u_out[3], long
   for (int it = 0; it < 200; ++it) {
     double P, cs2, T;
     eos_eval(o.eos, e, &P, &cs2, &T);
-    P += Pib;
+    if (Pib != 0.0) { P += Pib; if (P < 0.0) { P = 0.0; cs2 = 0.0; } }   // A32: total pressure max(P + Pi, 0)
     double g = M0 - Mabs * Mabs / (M0 + P) - e;
     if (std::fabs(g) <= 1e-15 * M0) break;
     if (g > 0) lo = e; else hi = e;
@@ -385,7 +386,7 @@ void rootfind(Oracle& o, const double M[4], double* e_out, double u_out[3], long
   if (e < o.e_floor) { e = o.e_floor; ++*nfloor; }
   double P, cs2, T;
   eos_eval(o.eos, e, &P, &cs2, &T);
-  P += Pib;
+  if (Pib != 0.0) P = std::max(P + Pib, 0.0);
   double v[3], v2 = 0;
   for (int a = 0; a < 3; ++a) { v[a] = Mi[a] / (M0 + P); v2 += v[a] * v[a]; }
   double gam = 1.0 / std::sqrt(1.0 - v2);

@@ -54,14 +54,14 @@ struct Layout {
 // 7.5 and 8.0.
 static int resolve_kernel(int kernel, int precision) { (void)precision; return kernel != 0 ? kernel : 4; }
 
-static bool make_layout(const hydro_grid* g, int precision, double eta_s, int kernel, Layout* L) {
+static bool make_layout(const hydro_grid* g, int precision, double eta_s, int kernel, Layout* L, bool ext = false) {
   if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;
   if (precision != 64 && precision != 32) return false;
   if ((long long)g->nx * g->ny * g->nz > (1ll << 36)) return false;
   // launch-grid limits of kernels 1/2 (gridDim.y, gridDim.z) and of the TMA coordinates of kernel 3
   if (g->nz > 65535 || g->ny > 8 * 65535 || g->nx > (1 << 30)) return false;
   L->elem = precision == 64 ? 8 : 4;
-  L->nf = eta_s > 0.0 ? 14 : 4;
+  L->nf = eta_s > 0.0 ? (ext ? 16 : 14) : 4;      // ext: the 16-word cell
   L->soa = resolve_kernel(kernel, precision) == 3 ? 1 : 0;
   if (L->soa) {
     const int per16 = 16 / (int)L->elem;
@@ -106,9 +106,10 @@ struct IoArgs {
   DiagDev* diag;
 };
 
-template <typename R, bool VISC>
+template <typename R, bool VISC, bool EXT = false>
 __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restrict__ T, const R* __restrict__ pi,
-                                                   R* __restrict__ st) {
+                                                   R* __restrict__ st, const R* __restrict__ Pib = nullptr,
+                                                   const R* __restrict__ nb = nullptr) {
   const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const bool active = cu < a.N;
   const long long cc = active ? cu : 0;
@@ -123,17 +124,20 @@ __global__ void __launch_bounds__(256) load_kernel(IoArgs<R> a, const R* __restr
   unsigned flags = 0;
   R e, ux, uy, un, P, cs2, g;
   // warp-uniform Newton with early exit (round 1 ran 64 fixed iterations here: 6.7 ms at 301x301x201)
-  rootfind_warp(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, P, cs2, ux, uy, un, g, flags);
+  // T is the full tensor, the root-find carries the bulk pressure (A28, A32)
+  const R Pb = (EXT && Pib) ? Pib[cc] : R(0);
+  rootfind_warp(a.eos, M[0], M[1], M[2], M[3], R(-1), 64, a.e_floor, a.v_max, e, P, cs2, ux, uy, un, g, flags, Pb, EXT);
   if (active) {
     st[c] = e; st[FS + c] = ux; st[2 * FS + c] = uy; st[3 * FS + c] = un;
     if (VISC) {
 #pragma unroll
       for (int m = 0; m < 10; ++m) st[(F_PI + m) * FS + c] = p[m];
     }
+    if (EXT) { st[(F_PI + 10) * FS + c] = Pb; st[(F_PI + 11) * FS + c] = nb ? nb[cc] : R(0); }
     // extended slots read by kernel 2
     R cx, cy, cn;
     signal_speeds3(g, ux, uy, un, cs2, cx, cy, cn);
-    R* __restrict__ sx = st + (VISC ? 14 : 4) * FS + c;
+    R* __restrict__ sx = st + (VISC ? (EXT ? 16 : 14) : 4) * FS + c;
     sx[X_P * FS] = P; sx[X_G * FS] = g;
     sx[X_CX * FS] = cx; sx[X_CY * FS] = cy; sx[X_CN * FS] = cn;
   } else {
@@ -164,6 +168,18 @@ __global__ void __launch_bounds__(256) read_kernel(IoArgs<R> a, const R* __restr
 }
 
 // pad (dir = 0: user -> internal) or unpad (dir = 1) three history fields
+// bulk pressure and net-baryon density of the state (fields 14, 15 of the 16-word cell)
+template <typename R>
+__global__ void __launch_bounds__(256) read_ext_kernel(IoArgs<R> a, const R* __restrict__ st, R* __restrict__ Pib,
+                                                       R* __restrict__ nb) {
+  const long long cu = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (cu >= a.N) return;
+  const int i = (int)(cu % a.nx), j = (int)((cu / a.nx) % a.ny), k = (int)(cu / ((long long)a.nx * a.ny));
+  const long long c = (long long)k * a.sz + (long long)j * a.sy + xoff(i, a.blk);
+  if (Pib) Pib[cu] = st[(F_PI + 10) * FS + c];
+  if (nb) nb[cu] = st[(F_PI + 11) * FS + c];
+}
+
 template <typename R>
 __global__ void __launch_bounds__(256) history_kernel(IoArgs<R> a, R* __restrict__ hist, R* __restrict__ user,
                                                       int dir) {
@@ -277,7 +293,8 @@ using namespace clv;
 struct hydro_ctx {
   hydro_grid grid;
   double dtau, tau0, eta_s;
-  int precision, visc, kernel, strict;
+  int precision, visc, kernel, strict, ext;
+  double zeta_s;
   double theta, e_floor, xi, v_max, lambda1_hat, c_tau;
   int root_iters;
   Layout L;
@@ -464,6 +481,7 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
   a.theta = (R)c->theta; a.e_floor = (R)c->e_floor; a.xi = (R)c->xi; a.v_max = (R)c->v_max;
   a.inv_5etas_hbarc = (R)(c->visc ? 1.0 / (c->c_tau * c->eta_s * kHbarc) : 0.0);
   a.inv_ctau = (R)(1.0 / c->c_tau); a.lam1 = (R)c->lambda1_hat;
+  a.zeta_over_eta = (R)((c->ext && c->visc) ? c->zeta_s / c->eta_s : 0.0);
   a.root_iters = c->root_iters;
   a.eos = eos_of<R>(c);
   a.diag = c->diag;
@@ -472,6 +490,13 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
 
 template <typename R, bool VISC, int MODE>
 int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
+  if constexpr (VISC) {
+    if (c->ext) {      // the 16-word cell runs in the per-cell fused kernel
+      launch_stage_fused<R, true, MODE, true>(a, c->stream);
+      c->launches += 1;
+      return cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+    }
+  }
   if (c->kernel == 4 && MODE != 0) {
     if constexpr (MODE != 0) {
       c->launches += 1;
@@ -566,13 +591,26 @@ int do_step(hydro_ctx* c) {
 }
 
 template <typename R>
-int do_load(hydro_ctx* c, const void* T, const void* pi, int mem) {
+int do_load(hydro_ctx* c, const void* T, const void* pi, int mem, const void* Pib = nullptr, const void* nb = nullptr) {
   const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
   const R* dT = static_cast<const R*>(T);
   const R* dpi = static_cast<const R*>(pi);
+  const R* dPib = static_cast<const R*>(Pib);
+  const R* dnb = static_cast<const R*>(nb);
   if (!c->visc) dpi = nullptr;
+  if (!(c->ext && c->visc)) { dPib = nullptr; dnb = nullptr; }
   if (mem == HYDRO_MEM_HOST) {
     R* stage = static_cast<R*>(c->buf[2]);
+    if (dPib) {
+      if (cudaMemcpyAsync(stage + 14 * N, Pib, (size_t)N * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        return HYDRO_ECUDA;
+      dPib = stage + 14 * N;
+    }
+    if (dnb) {
+      if (cudaMemcpyAsync(stage + 15 * N, nb, (size_t)N * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        return HYDRO_ECUDA;
+      dnb = stage + 15 * N;
+    }
     if (cudaMemcpyAsync(stage, T, (size_t)4 * N * sizeof(R), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
       return HYDRO_ECUDA;
     dT = stage;
@@ -585,15 +623,17 @@ int do_load(hydro_ctx* c, const void* T, const void* pi, int mem) {
   }
   if (cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) return HYDRO_ECUDA;
   c->cur = 0; c->prev = 1; c->step = 0;
-  const unsigned nb = (unsigned)((N + 255) / 256);
+  const unsigned nblk = (unsigned)((N + 255) / 256);
   if (c->L.soa) {
     SoaArgs<R> a = soa_args<R>(c);
-    if (c->visc) load_kernel_soa<R, true><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
-    else load_kernel_soa<R, false><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+    if (c->visc) load_kernel_soa<R, true><<<nblk, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+    else load_kernel_soa<R, false><<<nblk, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
   } else {
     IoArgs<R> a = io_args<R>(c);
-    if (c->visc) load_kernel<R, true><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
-    else load_kernel<R, false><<<nb, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+    if (c->visc && c->ext)
+      load_kernel<R, true, true><<<nblk, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]), dPib, dnb);
+    else if (c->visc) load_kernel<R, true><<<nblk, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
+    else load_kernel<R, false><<<nblk, 256, 0, c->stream>>>(a, dT, dpi, static_cast<R*>(c->buf[c->cur]));
   }
   c->launches += 1;
   if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
@@ -677,6 +717,30 @@ int do_history(hydro_ctx* c, void* user, int mem, int dir) {
   return HYDRO_OK;
 }
 
+// Pi and n of the current state to user arrays (device in place; host through buf X)
+template <typename R>
+int do_read_ext(hydro_ctx* c, void* Pib, void* nb, int mem) {
+  const long long N = (long long)c->grid.nx * c->grid.ny * c->grid.nz;
+  IoArgs<R> a = io_args<R>(c);
+  const unsigned nblk = (unsigned)((N + 255) / 256);
+  const R* st = static_cast<const R*>(c->buf[c->cur]);
+  R* dP = static_cast<R*>(Pib);
+  R* dn = static_cast<R*>(nb);
+  R* stage = static_cast<R*>(c->buf[2]);
+  if (mem == HYDRO_MEM_HOST) { dP = Pib ? stage : nullptr; dn = nb ? stage + N : nullptr; }
+  read_ext_kernel<R><<<nblk, 256, 0, c->stream>>>(a, st, dP, dn);
+  c->launches += 1;
+  if (cudaGetLastError() != cudaSuccess) return HYDRO_ECUDA;
+  if (mem == HYDRO_MEM_HOST) {
+    if (Pib && cudaMemcpyAsync(Pib, dP, (size_t)N * sizeof(R), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+    if (nb && cudaMemcpyAsync(nb, dn, (size_t)N * sizeof(R), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+      return HYDRO_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  }
+  return HYDRO_OK;
+}
+
 // freeze-out finder: bytes of one stored level; store the current state as level `which`
 static size_t frz_level_bytes(const hydro_grid* g, int precision) {
   const size_t N = (size_t)g->nx * g->ny * g->nz;
@@ -692,6 +756,13 @@ int frz_store_level(hydro_ctx* c, int which) {
 }  // namespace
 
 extern "C" {
+
+size_t hydro_workspace_bytes_ext(const hydro_grid* grid, int precision, double eta_over_s, int bulk_baryon) {
+  if (!bulk_baryon) return hydro_workspace_bytes(grid, precision, eta_over_s);
+  Layout L;
+  if (!(eta_over_s > 0.0) || !make_layout(grid, precision, eta_over_s, 2, &L, true)) return 0;
+  return L.total;
+}
 
 size_t hydro_workspace_bytes(const hydro_grid* grid, int precision, double eta_over_s) {
   // one figure for every kernel choice: the larger of the blocked (kernels 1/2) and the ghosted SoA (kernel 3) stores
@@ -711,7 +782,12 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
     const int kk = resolve_kernel(opts->kernel, opts->precision);
     if (kk != 2 && kk != 4) return HYDRO_EINVAL;
   }
-  if (!make_layout(grid, opts->precision, eta_over_s, opts->kernel, &L)) return HYDRO_EINVAL;
+  const bool ext = opts->bulk_baryon != 0;
+  if (ext) {      // viscous runs, blocked store (kernel 2), no strict Eq.53
+    const int kk = resolve_kernel(opts->kernel, opts->precision);
+    if (!(eta_over_s > 0.0) || (kk != 2 && kk != 4) || opts->strict_eq53 || !(opts->zeta_over_s >= 0.0)) return HYDRO_EINVAL;
+  }
+  if (!make_layout(grid, opts->precision, eta_over_s, ext ? 2 : opts->kernel, &L, ext)) return HYDRO_EINVAL;
   if (!(dtau > 0.0) || !(grid->dx > 0.0) || !(grid->dy > 0.0) || !(grid->deta > 0.0)) return HYDRO_EINVAL;
   if (grid->geometry != 0 && grid->geometry != 1) return HYDRO_EINVAL;
   if (grid->geometry == 0 && !(tau0 > 0.0)) return HYDRO_EINVAL;
@@ -749,6 +825,8 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
   c->kernel = resolve_kernel(opts->kernel, opts->precision);
   c->strict = opts->strict_eq53 ? 1 : 0;
+  c->ext = ext ? 1 : 0; c->zeta_s = ext ? opts->zeta_over_s : 0.0;
+  if (ext) c->kernel = 2;
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
   c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;
@@ -791,6 +869,18 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
 int hydro_load(hydro_ctx* c, const void* T, const void* pi, int mem) {
   if (!c || !T || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
   return c->precision == 64 ? do_load<double>(c, T, pi, mem) : do_load<float>(c, T, pi, mem);
+}
+
+int hydro_load_ext(hydro_ctx* c, const void* T, const void* pi, const void* Pi, const void* n_b, int mem) {
+  if (!c || !T || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
+  if (!c->ext) return HYDRO_ESTATE;
+  return c->precision == 64 ? do_load<double>(c, T, pi, mem, Pi, n_b) : do_load<float>(c, T, pi, mem, Pi, n_b);
+}
+
+int hydro_read_ext(hydro_ctx* c, void* Pi, void* n_b, int mem) {
+  if (!c || (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST)) return HYDRO_EINVAL;
+  if (!c->loaded || !c->ext) return HYDRO_ESTATE;
+  return c->precision == 64 ? do_read_ext<double>(c, Pi, n_b, mem) : do_read_ext<float>(c, Pi, n_b, mem);
 }
 
 int hydro_set_history(hydro_ctx* c, const void* u_prev, int mem) {

@@ -149,9 +149,13 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // slot0[m * 256] (INIT: first axis, "=" instead of "-=").  cfl = c_a h / Delta_a of the cell.  Shared by the per-cell
 // kernel (three axes) and the marching kernel (x and y; hydro_stage_march.cuh).  FSTR = element stride between the
 // fields of a point (32 in the blocked global store; the plane size of a shared-memory tile).
-template <typename R, bool USE_PI, int AX, bool INIT, int OX, int FSTR = FS, typename A>
-__device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ const (&pp)[5], R th2, R tf, R (&S)[14],
+// EXT: two more pi-like fields follow the ten pi components -- the bulk pressure Pi (Q = u^tau Pi,
+// F_a = u^a Pi, Eq.30) and the net-baryon density n (Q_N / tau = n u^tau, F_a / tau = n u^a, Eq.28; the factor tau is
+// applied by the stage tail) -- and Pi adds to the pressure in the T fields (A28).
+template <typename R, bool USE_PI, int AX, bool INIT, int OX, int FSTR = FS, bool EXT = false, typename A, int NS>
+__device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ const (&pp)[5], R th2, R tf, R (&S)[NS],
                                           R* slot0, R& cfl) {
+  constexpr int NTRIP = (EXT && USE_PI) ? 6 : 5;      // pi-like fields, two per trip
   const int o_ua = (1 + AX) * FSTR, o_ca = OX + (X_CX + AX) * FSTR;
   if (CLV_PFZ && USE_PI && AX == 2) {      // first pi trip of this axis: in flight behind the T-field part
 #pragma unroll
@@ -179,6 +183,7 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
 #pragma unroll
     for (int p = 0; p < 5; ++p) {
       Pp[p] = pp[p][OX + X_P * FSTR];
+      if (EXT && USE_PI) Pp[p] += pp[p][(F_PI + 10) * FSTR];      // P + Pi (A28)
       const R w = pp[p][0] + Pp[p];
       wq[p] = w * g[p]; wa[p] = w * ua[p];
     }
@@ -237,7 +242,7 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
       for (int p = 0; p < 5; ++p) { g2[p] = bc2((float)g[p]); ua2[p] = bc2((float)ua[p]); }
       const F2 cl2 = bc2((float)cl), ncr2 = bc2(-(float)cr), th22 = bc2((float)th2);
 #pragma unroll 1
-      for (int t = 0; t < 5; ++t) {
+      for (int t = 0; t < NTRIP; ++t) {
         F2 q[5], f[5];
         if (CLV_PFZ && AX == 2) {
 #pragma unroll
@@ -258,7 +263,7 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
       }
     } else {
 #pragma unroll 1
-    for (int t = 0; t < 5; ++t) {
+    for (int t = 0; t < NTRIP; ++t) {
       R qa[5], fa[5], qb[5], fb[5];
       if (CLV_PFZ && AX == 2) {      // next trip's fields on the four off-centre planes
 #pragma unroll
@@ -282,10 +287,15 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
   }
 }
 
-template <typename R, bool VISC, int MODE>
+// EXT: the 16-word cell of PAPER.md:614 -- fields 14 (bulk pressure Pi) and 15 (net-baryon density n)
+// follow the ten pi components; viscous runs only.
+template <typename R, bool VISC, int MODE, bool EXT = false>
 __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB)) stage_fused_kernel(const StageArgs<R> a) {
+  static_assert(!EXT || VISC, "the bulk / baryon extension rides on the viscous path");
   constexpr bool USE_PI = VISC && (MODE != 0);
-  constexpr int NF = VISC ? 14 : 4;                 // evolved fields of a buffer; extended slots follow
+  constexpr bool XT = EXT && USE_PI;                // the extension is active in this launch (not in the bootstrap)
+  constexpr int NPI = XT ? 12 : 10;                 // pi-like fields
+  constexpr int NF = VISC ? (EXT ? 16 : 14) : 4;    // evolved fields of a buffer; extended slots follow
   constexpr int OX = NF * FS;                       // element offset of the extended slots inside an x-block
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -300,11 +310,11 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
 
   // S_KT of the ten pi fields accumulates in thread-private shared-memory slots, so that the pi-field loop
   // can stay rolled (its ~200-instruction body then lives in the L0 instruction cache)
-  __shared__ R sS[USE_PI ? 10 * 256 : 1];
+  __shared__ R sS[USE_PI ? NPI * 256 : 1];
   const int tid = threadIdx.y * 32 + threadIdx.x;
-  R S[14];
+  R S[16];
 #pragma unroll
-  for (int m = 0; m < 14; ++m) S[m] = R(0);
+  for (int m = 0; m < 16; ++m) S[m] = R(0);
   R cfl0 = R(0), cfl1 = R(0), cfl2 = R(0);
   const R tf = a.milne ? a.tau : R(1);
   const R th2 = R(2) * a.theta;
@@ -320,13 +330,13 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
     const R* __restrict__ pp[5];
 #pragma unroll
     for (int p = 0; p < 5; ++p) pp[p] = in + idx[p];
-    if (ax == 0) axis_flux<R, USE_PI, 0, true, OX>(a, pp, th2, tf, S, &sS[tid], cfl0);
-    else if (ax == 1) axis_flux<R, USE_PI, 1, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl1);
-    else axis_flux<R, USE_PI, 2, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl2);
+    if (ax == 0) axis_flux<R, USE_PI, 0, true, OX, FS, XT>(a, pp, th2, tf, S, &sS[tid], cfl0);
+    else if (ax == 1) axis_flux<R, USE_PI, 1, false, OX, FS, XT>(a, pp, th2, tf, S, &sS[tid], cfl1);
+    else axis_flux<R, USE_PI, 2, false, OX, FS, XT>(a, pp, th2, tf, S, &sS[tid], cfl2);
   }
   if (USE_PI) {
 #pragma unroll
-    for (int m = 0; m < 10; ++m) S[4 + m] = sS[m * 256 + tid];
+    for (int m = 0; m < NPI; ++m) S[4 + m] = sS[m * 256 + tid];
   }
 
   // ---- cell-centre state (re-read after the flux loop: L1 hits, keeps the loop's register set small) ---
@@ -337,6 +347,7 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
   cc.P = pc[OX + X_P * FS];
 #pragma unroll
   for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
+  cc.Pi = XT ? pc[(F_PI + 10) * FS] : R(0); cc.nb = XT ? pc[(F_PI + 11) * FS] : R(0);
 
   // spatial rows of nabla~_mu u~^nu by central differences (A9); eta row divided by tau (Eq.22)
   R grad[4][4];
@@ -369,6 +380,7 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
     cn_.P = sn[OX + X_P * FS];
 #pragma unroll
     for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
+    cn_.Pi = XT ? sn[(F_PI + 10) * FS] : R(0); cn_.nb = XT ? sn[(F_PI + 11) * FS] : R(0);
   }
   R up3[3] = {R(0), R(0), R(0)};
   R gst = R(1);
@@ -385,7 +397,7 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
   unsigned flags = 0;
   Cell<R> nw;
   R cs2_new;
-  stage_update<R, VISC, MODE>(a, S, cc, cn_, grad, up3, gst, nw, cs2_new, flags);
+  stage_update<R, VISC, MODE, XT>(a, S, cc, cn_, grad, up3, gst, nw, cs2_new, flags, tf);
   const R* ut = cc.u;
   const R e_new = nw.e, P_new = nw.P, ux_new = nw.u[1], uy_new = nw.u[2], un_new = nw.u[3], g_new = nw.u[0];
   const R* pnew = nw.pi;
@@ -402,6 +414,7 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
       if (VISC) {
 #pragma unroll
         for (int m = 0; m < 10; ++m) out[(F_PI + m) * FS] = pnew[m];
+        if (XT) { out[(F_PI + 10) * FS] = nw.Pi; out[(F_PI + 11) * FS] = nw.nb; }
         if (MODE == 1) a.gstar[cg] = gst;
       }
       out[OX + X_P * FS] = P_new; out[OX + X_G * FS] = g_new;
@@ -433,11 +446,11 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MINB32 : CLV_MINB))
   }
 }
 
-template <typename R, bool VISC, int MODE>
+template <typename R, bool VISC, int MODE, bool EXT = false>
 void launch_stage_fused(const StageArgs<R>& a, cudaStream_t stream) {
   dim3 block(32, 8, 1);
   dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, a.nz);
-  stage_fused_kernel<R, VISC, MODE><<<grid, block, 0, stream>>>(a);
+  stage_fused_kernel<R, VISC, MODE, EXT><<<grid, block, 0, stream>>>(a);
 }
 
 }  // namespace clv

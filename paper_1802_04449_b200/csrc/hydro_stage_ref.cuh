@@ -31,6 +31,7 @@ struct StageArgs {
   R theta, e_floor, xi, v_max;
   R inv_5etas_hbarc;     // 1/(c_tau (eta_v/s) hbarc), c_tau = 5 unless set (tau_pi = c_tau eta_v/(T s))
   R inv_ctau, lam1;      // 1/c_tau; lambda1_hat (lambda_1 = lambda1_hat / e)
+  R zeta_over_eta;       // (zeta/s)/(eta_v/s); 0 without the extension
   int root_iters;
   const R* in;           // state whose 13-point star is read
   const R* sn;           // MODE 2: state n (cell centre only)

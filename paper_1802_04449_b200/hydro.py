@@ -16,7 +16,8 @@ from . import build as _build
 HYDRO_MEM_DEVICE, HYDRO_MEM_HOST = 0, 1
 SYMBOLS = ["hydro_workspace_bytes", "hydro_create", "hydro_load", "hydro_set_history", "hydro_read_history",
            "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_kernel", "hydro_destroy", "hydro_strerror",
-           "hydro_freezeout_bytes", "hydro_freezeout_begin", "hydro_freezeout_slab", "hydro_freezeout_run"]
+           "hydro_freezeout_bytes", "hydro_freezeout_begin", "hydro_freezeout_slab", "hydro_freezeout_run",
+           "hydro_workspace_bytes_ext", "hydro_load_ext", "hydro_read_ext"]
 
 
 class hydro_grid(Structure):
@@ -33,7 +34,8 @@ class hydro_opts(Structure):
     _fields_ = [("precision", c_int), ("minmod_theta", c_double), ("e_floor", c_double),
                 ("pi_limit_xi", c_double), ("v_max", c_double), ("root_iters", c_int), ("kernel", c_int),
                 ("stream", c_void_p), ("workspace", c_void_p), ("workspace_bytes", c_size_t),
-                ("lambda1_hat", c_double), ("tau_pi_coeff", c_double), ("strict_eq53", c_int)]
+                ("lambda1_hat", c_double), ("tau_pi_coeff", c_double), ("strict_eq53", c_int),
+                ("bulk_baryon", c_int), ("zeta_over_s", c_double)]
 
 
 class hydro_diag_t(Structure):
@@ -83,6 +85,12 @@ def load_library():
     lib.hydro_freezeout_run.restype = c_int
     lib.hydro_freezeout_run.argtypes = [c_void_p, c_int, c_int, c_void_p, c_void_p, c_longlong, POINTER(c_longlong),
                                         POINTER(c_int)]
+    lib.hydro_workspace_bytes_ext.restype = c_size_t
+    lib.hydro_workspace_bytes_ext.argtypes = [POINTER(hydro_grid), c_int, c_double, c_int]
+    lib.hydro_load_ext.restype = c_int
+    lib.hydro_load_ext.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int]
+    lib.hydro_read_ext.restype = c_int
+    lib.hydro_read_ext.argtypes = [c_void_p, c_void_p, c_void_p, c_int]
     lib.hydro_destroy.restype = None
     lib.hydro_destroy.argtypes = [c_void_p]
     lib.hydro_strerror.restype = ctypes.c_char_p
@@ -122,7 +130,8 @@ class Hydro:
 
     def __init__(self, nx, ny, nz, dx, dy, deta, dtau, tau0, eos, eta_over_s, bc=(0, 0, 0), geometry=0,
                  precision=64, minmod_theta=1.1, e_floor=1e-7, pi_limit_xi=1.0, v_max=0.0, root_iters=0,
-                 kernel=0, device="cuda:0", stream=None, lambda1_hat=0.0, tau_pi_coeff=0.0, strict_eq53=0):
+                 kernel=0, device="cuda:0", stream=None, lambda1_hat=0.0, tau_pi_coeff=0.0, strict_eq53=0,
+                 bulk_baryon=0, zeta_over_s=0.0):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -137,7 +146,8 @@ class Hydro:
         self.N = nx * ny * nz
         self.viscous = eta_over_s > 0
         self.grid = make_grid(nx, ny, nz, dx, dy, deta, bc, geometry)
-        nbytes = workspace_bytes(self.grid, precision, eta_over_s)
+        self.bulk_baryon = int(bulk_baryon)
+        nbytes = int(self._lib.hydro_workspace_bytes_ext(byref(self.grid), precision, eta_over_s, self.bulk_baryon))
         if nbytes == 0:
             raise HydroError("hydro_workspace_bytes: invalid grid / precision")
         with torch.cuda.device(self.device):
@@ -158,6 +168,7 @@ class Hydro:
         o.root_iters, o.kernel = root_iters, kernel
         o.lambda1_hat, o.tau_pi_coeff = lambda1_hat, tau_pi_coeff
         o.strict_eq53 = int(strict_eq53)
+        o.bulk_baryon, o.zeta_over_s = self.bulk_baryon, float(zeta_over_s)
         o.stream = c_void_p(self.stream.cuda_stream)
         o.workspace, o.workspace_bytes = c_void_p(aligned), nbytes
         with torch.cuda.device(self.device):
@@ -233,6 +244,25 @@ class Hydro:
         return dict(tau=d.tau, step=int(d.step), cfl=tuple(d.cfl), e_max=d.e_max, floored=int(d.n_floor),
                     clamped=int(d.n_clamp), pi_limited=int(d.n_pi_limited), nan=int(d.n_nan),
                     root_unconverged=int(d.n_root_unconverged), warn=warn)
+
+    # -- bulk pressure and net-baryon density (contexts created with bulk_baryon=1) ---------
+    def load_ext(self, T, pi=None, Pi=None, nb=None):
+        """hydro_load_ext: T^{tau mu} [4,...] (full tensor incl. Pi), pi [10,...], Pi [...], n [...]; all in one memory space."""
+        pT, mT, k1 = self._ptr(T, 4)
+        pp, mp, k2 = self._ptr(pi, 10)
+        pP, mP, k3 = self._ptr(Pi, 1)
+        pn, mn, k4 = self._ptr(nb, 1)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_load_ext(self._h, pT, pp, pP, pn, mT), "hydro_load_ext")
+
+    def read_ext(self, host=True):
+        """(Pi, n) of the current state, each [nz, ny, nx]."""
+        Pi, nb = self._empty(self.shape, host), self._empty(self.shape, host)
+        pP, mP, _ = self._ptr(Pi, 1, writable=True)
+        pn, mn, _ = self._ptr(nb, 1, writable=True)
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_read_ext(self._h, pP, pn, mP), "hydro_read_ext")
+        return Pi, nb
 
     # -- freeze-out hypersurface (SURVEY 8(f)-1) -------------------------------------------------
     def freezeout_begin(self, e_frz, capacity):

@@ -93,6 +93,7 @@ def test_create_refuses_a_host_workspace():
     """hydro_create checks the workspace with cudaPointerGetAttributes: host memory is HYDRO_EINVAL, not a fault in a
     kernel later."""
     import numpy as np
+    from ctypes import byref, c_void_p
     from paper_1802_04449_b200 import hydro
     lib = hydro.load_library()
     g = hydro.make_grid(8, 8, 8, 0.1, 0.1, 0.1)
