@@ -174,7 +174,12 @@ int hydro_read(hydro_ctx *ctx, void *e, void *u, void *pi, int mem);
  *   Returns HYDRO_ENOMEM when n_total exceeds capacity (the elements that did not fit are dropped), HYDRO_ESTATE before
  *   hydro_freezeout_begin.
  * hydro_freezeout_run: repeats { hydro_step(steps_per_slab); hydro_freezeout_slab } until no hot cell is left or
- *   max_slabs slabs are done; *n_slabs = slabs done. */
+ *   max_slabs slabs are done; *n_slabs = slabs done.
+ *
+ * hydro_eos_e_of_temperature: the energy density at which the EoS (rule A16: linear in e inside a bracket) has temperature T (GeV),
+ *   so that a constant-T_f surface is the constant-e_frz surface at e_frz = e(T_f).  Host arithmetic, no device needed.
+ *   HYDRO_EINVAL for a bad table or a table whose T does not increase with e. */
+int hydro_eos_e_of_temperature(const hydro_eos *eos, double T, double *e_out);
 size_t hydro_freezeout_bytes(const hydro_grid *grid, int precision);
 int hydro_freezeout_begin(hydro_ctx *ctx, void *workspace, size_t workspace_bytes, double e_frz);
 int hydro_freezeout_slab(hydro_ctx *ctx, long long *keys, double *rows, long long capacity,

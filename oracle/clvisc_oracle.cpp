@@ -215,7 +215,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
   if (ext) { SX[0].assign(N, 0.0); SX[1].assign(N, 0.0); }
 
   // step 1-2: EoS and conserved variables at every cell
-#pragma omp parallel for
+#pragma omp parallel for if (N >= 2048)
   for (size_t c = 0; c < N; ++c) {
     double Tf[4][4], ut[4];
     eos_eval(o.eos, s.e[c], &pt.P[c], &pt.cs2[c], &pt.T[c]);
@@ -229,7 +229,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
   for (int a = 0; a < 3; ++a) {
     double cflmax = 0.0;
     const double scale = (a == 2 && milne) ? 1.0 / (tau * o.d[2]) : 1.0 / o.d[a];
-#pragma omp parallel for reduction(max : cflmax)
+#pragma omp parallel for if (N >= 2048) reduction(max : cflmax)
     for (size_t c = 0; c < N; ++c) {
       double Tf[4][4], ut[4];
       frame_tensor(o, s, c, use_pi, pt.P[c], Tf, ut);
@@ -242,7 +242,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
       cflmax = std::max(cflmax, pt.c[c] * o.dtau * scale);
     }
     if (cfl_out) cfl_out[a] = cflmax;
-#pragma omp parallel for
+#pragma omp parallel for if (N >= 2048)
     for (size_t c = 0; c < N; ++c) {
       int i = int(c % o.nx), j = int((c / o.nx) % o.ny), k = int(c / (size_t(o.nx) * o.ny));
       size_t m2 = o.nb(i, j, k, a, -2), m1 = o.nb(i, j, k, a, -1);
@@ -259,7 +259,7 @@ void rhs(const Oracle& o, const State& s, bool use_pi, const std::vector<double>
   }
 
   // step 6-7: geometric source of T (Eq.31, sign A1), velocity gradients, IS source (Eq.33, A1, A2)
-#pragma omp parallel for
+#pragma omp parallel for if (N >= 2048)
   for (size_t c = 0; c < N; ++c) {
     int i = int(c % o.nx), j = int((c / o.nx) % o.ny), k = int(c / (size_t(o.nx) * o.ny));
     double Tf[4][4], ut[4];
@@ -442,7 +442,7 @@ void bootstrap_history(Oracle& o) {
   rhs(o, s, false, nullptr, o.tau0, ST, SP, nullptr);
   double tf0 = milne ? o.tau0 : 1.0, tf1 = milne ? o.tau0 + o.dtau : 1.0;
   long dummy1 = 0, dummy2 = 0;
-#pragma omp parallel for reduction(+ : dummy1, dummy2)
+#pragma omp parallel for if (N >= 2048) reduction(+ : dummy1, dummy2)
   for (size_t c = 0; c < N; ++c) {
     double QT[4], M[4], e1, u1[3];
     conserved_T(o, s, c, false, tf0, QT);
@@ -464,7 +464,7 @@ void step_once(Oracle& o) {
   // ---- stage 1 at tau_n -------------------------------------------------------------------
   std::vector<double> dtu[4], gstar(N);
   for (int m = 0; m < 4; ++m) dtu[m].resize(N);
-#pragma omp parallel for
+#pragma omp parallel for if (N >= 2048)
   for (size_t c = 0; c < N; ++c) {
     double us[3], g2 = 1.0, gs2 = 1.0;
     for (int a = 0; a < 3; ++a) {
@@ -489,7 +489,7 @@ void step_once(Oracle& o) {
   std::vector<double> Pi1, nb1, QNn;   // 8(f)-3: Pi', n' and Q_N^n
   if (ext) { Pi1.assign(N, 0.0); nb1.assign(N, 0.0); QNn.assign(N, 0.0); }
   long nfl = 0, ncl = 0, nli = 0, nbl = 0;   // event counters of this step (summed over the flat cell loops)
-#pragma omp parallel for reduction(+ : nfl, ncl, nli, nbl)
+#pragma omp parallel for if (N >= 2048) reduction(+ : nfl, ncl, nli, nbl)
   for (size_t c = 0; c < N; ++c) {
     double QT[4], pp[10] = {0}, M[4], uu[3];
     conserved_T(o, sn, c, visc, tf_n, QT);
@@ -515,7 +515,7 @@ void step_once(Oracle& o) {
   }
 
   // ---- stage 2 at tau_{n+1} ---------------------------------------------------------------
-#pragma omp parallel for
+#pragma omp parallel for if (N >= 2048)
   for (size_t c = 0; c < N; ++c) {
     double g2 = 1.0, g12 = 1.0;
     for (int a = 0; a < 3; ++a) { g2 += o.u[a][c] * o.u[a][c]; g12 += u1[a][c] * u1[a][c]; }
@@ -534,7 +534,7 @@ void step_once(Oracle& o) {
   std::vector<double> pinew[10];
   for (int m = 0; m < 10; ++m) pinew[m].assign(N, 0.0);
   if (visc) {
-#pragma omp parallel for
+#pragma omp parallel for if (N >= 2048)
     for (size_t c = 0; c < N; ++c) {
       double gn = std::sqrt(1.0 + o.u[0][c] * o.u[0][c] + o.u[1][c] * o.u[1][c] + o.u[2][c] * o.u[2][c]);
       double g1 = std::sqrt(1.0 + u1[0][c] * u1[0][c] + u1[1][c] * u1[1][c] + u1[2][c] * u1[2][c]);
@@ -551,7 +551,7 @@ void step_once(Oracle& o) {
       rhs(o, s1b, true, dtu, tau_1, ST1, SPdummy, nullptr);
     }
   }
-#pragma omp parallel for reduction(+ : nfl, ncl, nli, nbl)
+#pragma omp parallel for if (N >= 2048) reduction(+ : nfl, ncl, nli, nbl)
   for (size_t c = 0; c < N; ++c) {
     double QT1[4], M[4], pp[10], en, uu[3];
     conserved_T(o, s1, c, visc, tf_1, QT1);
@@ -630,7 +630,7 @@ int oracle_load_ext(void* h, const double* T, const double* pi, const double* Pi
   const bool ext = o.ext && o.viscous();
   if (ext) { o.Pi.assign(N, 0.0); o.nB.assign(N, 0.0); }
   long nfl = 0, ncl = 0;
-#pragma omp parallel for reduction(+ : nfl, ncl)
+#pragma omp parallel for if (N >= 2048) reduction(+ : nfl, ncl)
   for (size_t c = 0; c < N; ++c) {
     double M[4], uu[3];
     for (int m = 0; m < 10; ++m) o.pi[m][c] = (pi && o.viscous()) ? pi[m * N + c] : 0.0;

@@ -915,6 +915,27 @@ int hydro_read(hydro_ctx* c, void* e, void* u, void* pi, int mem) {
 
 // ---- freeze-out hypersurface (hydro_freezeout.cuh) ----------------------------------------------------
 
+// Freeze-out at constant temperature ("constant freeze-out temperature T_f or constant freeze-out energy
+// density e_f"): T(e) of the EoS rule A16 is monotone, so T_f is an e_f.  Host arithmetic only (no device needed).
+int hydro_eos_e_of_temperature(const hydro_eos* eos, double T, double* e_out) {
+  if (!eos || !e_out || !(T > 0.0) || !(eos->c_sb > 0.0)) return HYDRO_EINVAL;
+  if (eos->kind == 0) { *e_out = eos->c_sb * kHbarc * std::pow(T / kHbarc, 4.0); return HYDRO_OK; }
+  if (eos->kind != 1 || eos->n < 2 || !eos->T || !(eos->e_min > 0.0) || !(eos->e_max > eos->e_min)) return HYDRO_EINVAL;
+  const int n = eos->n;
+  auto node = [&](int k) { return eos->e_min * std::pow(eos->e_max / eos->e_min, double(k) / double(n - 1)); };
+  if (T <= eos->T[0]) { *e_out = eos->e_min * std::pow(T / eos->T[0], 4.0); return HYDRO_OK; }            // T = T_0 (e/e_min)^{1/4}
+  if (T >= eos->T[n - 1]) { *e_out = eos->e_max * std::pow(T / eos->T[n - 1], 4.0); return HYDRO_OK; }
+  int lo = 0, hi = n - 1;      // T[lo] <= T < T[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) / 2;
+    if (eos->T[mid] <= T) lo = mid; else hi = mid;
+  }
+  const double e0 = node(lo), e1 = node(lo + 1), dT = eos->T[lo + 1] - eos->T[lo];
+  if (!(dT > 0.0)) return HYDRO_EINVAL;      // T must increase with e for the inverse to exist
+  *e_out = e0 + (T - eos->T[lo]) * (e1 - e0) / dT;
+  return HYDRO_OK;
+}
+
 size_t hydro_freezeout_bytes(const hydro_grid* grid, int precision) {
   if (!grid || grid->nx < 1 || grid->ny < 1 || grid->nz < 1 || (precision != 64 && precision != 32)) return 0;
   return 256 + 2 * frz_level_bytes(grid, precision);

@@ -15,9 +15,11 @@
 //     fields (65.7 KB fp64, two blocks per SM), filled with cp.async one plane ahead, behind the stage tail of the
 //     previous plane -- the paper's local-memory block, which its GPU had no room for.  The
 //     boundary rule a11 is applied to the source index of the copy, so the tile needs no special cases;
+//   * fp32 only: the raw words of plane p are stashed in tensor memory next to the pipeline state, so the next eta_s step
+//     reads plane p-1 from there and only ONE plane per step comes from global memory (fp64: measured slower, off);
 //   * one block barrier per plane (two with the tile) keeps the 8 warps of a block on the same instruction-cache lines
 //     of the ~90 KB loop body: without it "no instruction" stalls are 1.8 warps per issue, with it 0.19.
-// Measured at 301x301x201 (profiles/round2_bench.md): 11.8 ms per step fp64, 6.3 ms fp32 (kernel 2: 14.4 / 7.5).
+// Measured at 301x301x201 (profiles/round2_bench.md): 11.8 ms per step fp64, 6.1 ms fp32 (kernel 2: 14.4 / 7.5).
 // Citations: KT scheme PAPER.md:193-213 (Eq.40-44); RK2 :225-239 (Eq.49-54).
 #pragma once
 #include "hydro_stage_fused.cuh"
@@ -55,21 +57,100 @@ __device__ __forceinline__ void cp_async_elem(float* dst_smem, const float* src)
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
 }
 
-// columns of tensor memory a block allocates: 8 warps share 4 lane quadrants, 3 kept values per evolved field
+// ---- tensor memory as the per-thread store of the eta_s pipeline --------------------------------------------------------
+// Per thread (one TMEM lane segment, 32x32b shape): for each of the 14 evolved fields FOUR values
+//   [Q^l, F^l of cell p-2;  2H of face p-5/2;  the field's raw value at plane p-1 (the "stash")]
+// and three more stashed words of plane p-1 (u~^tau, P, c_eta): 59 values = 118 (fp64) / 59 (fp32) columns; 8 warps share
+// 4 lane quadrants, so a block allocates 256 / 128 columns.  The stash means that an eta_s step reads only ONE plane
+// from global memory (plane p; p-1 comes from here, p-2 from the shared-memory tile).
+// Measured at 301x301x201 (profiles/round2_bench.md): fp32 6.21 -> 6.06 ms per step, fp64 11.79 -> 12.03 (the TMEM round
+// trips cost the fp64 kernel more than the L1 misses they replace), so the stash is on in fp32 only.
+#ifndef CLV_MARCH_STASH
+#define CLV_MARCH_STASH 2      // 0 off, 1 on, 2 on in fp32 only
+#endif
+template <int N> struct TmWords { unsigned w[N]; };
+__device__ __forceinline__ void tm_ld_x(unsigned addr, TmWords<2>& v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(v.w[0]), "=r"(v.w[1]) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tm_ld_x(unsigned addr, TmWords<1>& v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v.w[0]) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tm_ld_x(unsigned addr, TmWords<4>& v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(v.w[0]), "=r"(v.w[1]), "=r"(v.w[2]), "=r"(v.w[3]) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tm_ld_x(unsigned addr, TmWords<8>& v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(v.w[0]), "=r"(v.w[1]), "=r"(v.w[2]), "=r"(v.w[3]), "=r"(v.w[4]), "=r"(v.w[5]), "=r"(v.w[6]), "=r"(v.w[7])
+               : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tm_ld_x(unsigned addr, TmWords<16>& v) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+               : "=r"(v.w[0]), "=r"(v.w[1]), "=r"(v.w[2]), "=r"(v.w[3]), "=r"(v.w[4]), "=r"(v.w[5]), "=r"(v.w[6]), "=r"(v.w[7]),
+                 "=r"(v.w[8]), "=r"(v.w[9]), "=r"(v.w[10]), "=r"(v.w[11]), "=r"(v.w[12]), "=r"(v.w[13]), "=r"(v.w[14]), "=r"(v.w[15])
+               : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void tm_st_x(unsigned addr, const TmWords<1>& v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(addr), "r"(v.w[0]) : "memory");
+}
+__device__ __forceinline__ void tm_st_x(unsigned addr, const TmWords<2>& v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(addr), "r"(v.w[0]), "r"(v.w[1]) : "memory");
+}
+__device__ __forceinline__ void tm_st_x(unsigned addr, const TmWords<4>& v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.w[0]), "r"(v.w[1]),
+               "r"(v.w[2]), "r"(v.w[3]) : "memory");
+}
+__device__ __forceinline__ void tm_st_x(unsigned addr, const TmWords<8>& v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(addr), "r"(v.w[0]),
+               "r"(v.w[1]), "r"(v.w[2]), "r"(v.w[3]), "r"(v.w[4]), "r"(v.w[5]), "r"(v.w[6]), "r"(v.w[7]) : "memory");
+}
+__device__ __forceinline__ void tm_st_x(unsigned addr, const TmWords<16>& v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+               ::"r"(addr), "r"(v.w[0]), "r"(v.w[1]), "r"(v.w[2]), "r"(v.w[3]), "r"(v.w[4]), "r"(v.w[5]), "r"(v.w[6]), "r"(v.w[7]),
+               "r"(v.w[8]), "r"(v.w[9]), "r"(v.w[10]), "r"(v.w[11]), "r"(v.w[12]), "r"(v.w[13]), "r"(v.w[14]), "r"(v.w[15])
+               : "memory");
+}
+// the wait ties the loaded registers to a point after it (no use can be scheduled before the wait)
+template <int N> __device__ __forceinline__ void tm_wait_ld_x(TmWords<N>& v) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < N; ++i) asm volatile("" : "+r"(v.w[i]));
+}
+template <int N> __device__ __forceinline__ double tm_val(const TmWords<N>& v, int i, double) {
+  return __hiloint2double((int)v.w[2 * i + 1], (int)v.w[2 * i]);
+}
+template <int N> __device__ __forceinline__ float tm_val(const TmWords<N>& v, int i, float) { return __uint_as_float(v.w[i]); }
+template <int N> __device__ __forceinline__ void tm_set(TmWords<N>& v, int i, double x) {
+  v.w[2 * i] = (unsigned)__double2loint(x); v.w[2 * i + 1] = (unsigned)__double2hiint(x);
+}
+template <int N> __device__ __forceinline__ void tm_set(TmWords<N>& v, int i, float x) { v.w[i] = __float_as_uint(x); }
+
 template <typename R>
 struct MarchTmem {
   static constexpr int W = sizeof(R) / 4;
-  static constexpr int COLS_PER_THREAD = 14 * 3 * W;                      // 84 (fp64) / 42 (fp32)
+  static constexpr int NVAL = 14 * 4 + 3;
+  static constexpr int COLS_PER_THREAD = NVAL * W;                       // 118 (fp64) / 59 (fp32)
   static constexpr int ALLOC_COLS = 2 * COLS_PER_THREAD <= 128 ? 128 : 256;
   unsigned base;
   __device__ __forceinline__ void init(unsigned tmem_base, int warp) {
     base = tmem_base + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)((warp >> 2) * COLS_PER_THREAD);
   }
-  __device__ __forceinline__ void get(int f, R& ql, R& fl, R& h) const { tm_ld3(base + f * 3 * W, ql, fl, h); }
+  __device__ __forceinline__ unsigned field(int f) const { return base + (unsigned)(f * 4 * W); }      // 4 values of field f
+  __device__ __forceinline__ unsigned stash(int f) const { return base + (unsigned)((f * 4 + 3) * W); }
+  __device__ __forceinline__ unsigned aux(int i) const { return base + (unsigned)((56 + i) * W); }   // 0 u~^tau, 1 P, 2 c_eta
+  // three-value access (the build without the stash, CLV_MARCH_STASH = 0)
+  __device__ __forceinline__ void get(int f, R& ql, R& fl, R& h) const { tm_ld3(field(f), ql, fl, h); }
   __device__ __forceinline__ void put(int f, R ql, R fl, R h) const {
-    tm_st(base + f * 3 * W, ql); tm_st(base + (f * 3 + 1) * W, fl); tm_st(base + (f * 3 + 2) * W, h);
+    tm_st(field(f), ql); tm_st(field(f) + W, fl); tm_st(field(f) + 2 * W, h);
   }
 };
+template <int N, int M> __device__ __forceinline__ void tm_wait_ld_x(TmWords<N>& a, TmWords<M>& b) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < N; ++i) asm volatile("" : "+r"(a.w[i]));
+#pragma unroll
+  for (int i = 0; i < M; ++i) asm volatile("" : "+r"(b.w[i]));
+}
 
 #ifndef CLV_MARCH_MINB32
 #define CLV_MARCH_MINB32 3      // fp32 blocks per SM: 3 (<= 85 registers) measured 6.28 ms per step against 6.8 with 2
@@ -147,6 +228,17 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
   const R sc_pi = R(0.5) * a.scale[2], sc_T = sc_pi * tf;
   R cflm0 = R(0), cflm1 = R(0), cflm2 = R(0), emax = R(0);
 
+  constexpr bool STASH = (CLV_MARCH_STASH == 1) || (CLV_MARCH_STASH == 2 && sizeof(R) == 4);
+  if constexpr (STASH) {   // the stash starts with plane kc0-1
+    const R* __restrict__ qm = in + (long long)bmap(kc0 - 1, a.nz, a.bc[2]) * a.sz + col;
+    TmWords<Priv::W> v;
+#pragma unroll
+    for (int m = 0; m < NF; ++m) { tm_set(v, 0, qm[m * FS]); tm_st_x(priv.stash(m), v); }
+    tm_set(v, 0, qm[OX + X_G * FS]); tm_st_x(priv.aux(0), v);
+    tm_set(v, 0, qm[OX + X_P * FS]); tm_st_x(priv.aux(1), v);
+    tm_set(v, 0, qm[OX + X_CN * FS]); tm_st_x(priv.aux(2), v);
+    tm_wait_st();
+  }
   for (int p = kc0; p <= kc1 + 1; ++p) {
     const int k = p - 2;
     const bool centre = p >= kc0 + 2;                      // block-uniform
@@ -189,7 +281,107 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
     for (int m = 0; m < 14; ++m) S[m] = R(0);
     R cfl2;
     // ---- eta_s pipeline step: slope of cell p-1, face p-3/2, flux difference of cell p-2 ---------------------------
-    {
+    if constexpr (STASH) {
+      // plane p from global memory, plane p-1 from the tensor-memory stash, plane p-2 from the tile
+      constexpr int TW = Priv::W;
+      using W1 = TmWords<TW>;
+      using W4 = TmWords<4 * TW>;
+      using W8 = TmWords<8 * TW>;
+#define P2_LD(m) (ETILE ? town[(m) * MT_FST] : q2[(m) * FS])
+      R g[3], ua[3], Pp[3], e3[3];
+      g[0] = P2_LD(NF + X_G); ua[0] = P2_LD(3); Pp[0] = P2_LD(NF + X_P); e3[0] = P2_LD(0);
+      const R c2 = P2_LD(NF + X_CN);
+      g[2] = q0[OX + X_G * FS]; ua[2] = q0[3 * FS]; Pp[2] = q0[OX + X_P * FS]; e3[2] = q0[0];
+      const R cnew = q0[OX + X_CN * FS];
+      R c1;
+      {
+        W1 a0, a1, a2; W4 f0; W1 s3;
+        tm_ld_x(priv.aux(0), a0); tm_ld_x(priv.aux(1), a1); tm_ld_x(priv.aux(2), a2);
+        tm_ld_x(priv.stash(0), s3);      // (reused below) e of plane p-1
+        tm_wait_ld_x(a0, a1); tm_wait_ld_x(a2, s3);
+        g[1] = tm_val(a0, 0, R()); Pp[1] = tm_val(a1, 0, R()); c1 = tm_val(a2, 0, R()); e3[1] = tm_val(s3, 0, R());
+        tm_ld_x(priv.stash(3), s3);
+        tm_wait_ld_x(s3);
+        ua[1] = tm_val(s3, 0, R());
+        (void)f0;
+      }
+      const R cface = max_(c2, c1);
+      cfl2 = c2 * a.h * a.scale[2];
+      {
+        R wq[3], wa[3];
+#pragma unroll
+        for (int t = 0; t < 3; ++t) {
+          const R w = e3[t] + Pp[t];
+          wq[t] = w * g[t]; wa[t] = w * ua[t];
+        }
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+          const int o_t = F_PI + mu, o_a = F_PI + c_pidx[3][mu];
+          W4 k4; W1 st, sa;
+          tm_ld_x(priv.field(mu), k4);
+          if (USE_PI) { tm_ld_x(priv.stash(o_t), st); tm_ld_x(priv.stash(o_a), sa); tm_wait_ld_x(st, sa); }
+          tm_wait_ld_x(k4);
+          const R raw_p = q0[mu * FS];      // field mu at plane p (e for mu = 0): the new stash
+          R um[3];
+          um[0] = mu == 0 ? g[0] : P2_LD(mu);
+          um[1] = mu == 0 ? g[1] : tm_val(k4, 3, R());
+          um[2] = mu == 0 ? g[2] : raw_p;
+          R q[3], f[3];
+#pragma unroll
+          for (int t = 0; t < 3; ++t) {
+            q[t] = wq[t] * um[t] - (mu == 0 ? Pp[t] : R(0));
+            f[t] = wa[t] * um[t] + (mu == 3 ? Pp[t] : R(0));
+          }
+          if (USE_PI) {
+            q[0] += P2_LD(o_t); f[0] += P2_LD(o_a);
+            q[1] += tm_val(st, 0, R()); f[1] += tm_val(sa, 0, R());
+            q[2] += q0[o_t * FS]; f[2] += q0[o_a * FS];
+          }
+          const R QLk = tm_val(k4, 0, R()), FLk = tm_val(k4, 1, R()), Hk = tm_val(k4, 2, R());
+          R QL1, QR1, FL1, FR1;
+          lr(q[0], q[1], q[2], th2, QL1, QR1);
+          lr(f[0], f[1], f[2], th2, FL1, FR1);
+          const R Hn = face2(QLk, FLk, QR1, FR1, cface);
+          S[mu] = -(Hn - Hk) * sc_T;
+          W4 n4;
+          tm_set(n4, 0, QL1); tm_set(n4, 1, FL1); tm_set(n4, 2, Hn); tm_set(n4, 3, raw_p);
+          tm_st_x(priv.field(mu), n4);
+        }
+        // the three derived words of plane p
+        W1 a0, a1, a2;
+        tm_set(a0, 0, g[2]); tm_set(a1, 0, Pp[2]); tm_set(a2, 0, cnew);
+        tm_st_x(priv.aux(0), a0); tm_st_x(priv.aux(1), a1); tm_st_x(priv.aux(2), a2);
+      }
+      if (USE_PI) {
+        R* slot = &sS[tid];
+#pragma unroll 1
+        for (int t = 0; t < 5; ++t) {
+          const int fa = F_PI + 2 * t;
+          W8 k8;
+          tm_ld_x(priv.field(fa), k8);
+          const R va0 = P2_LD(fa), vb0 = P2_LD(fa + 1), va2 = q0[fa * FS], vb2 = q0[(fa + 1) * FS];
+          tm_wait_ld_x(k8);
+          const R va1 = tm_val(k8, 3, R()), vb1 = tm_val(k8, 7, R());
+          R QL1, QR1, FL1, FR1;
+          W8 n8;
+          lr(g[0] * va0, g[1] * va1, g[2] * va2, th2, QL1, QR1);
+          lr(ua[0] * va0, ua[1] * va1, ua[2] * va2, th2, FL1, FR1);
+          const R Hna = face2(tm_val(k8, 0, R()), tm_val(k8, 1, R()), QR1, FR1, cface);
+          tm_set(n8, 0, QL1); tm_set(n8, 1, FL1); tm_set(n8, 2, Hna); tm_set(n8, 3, va2);
+          lr(g[0] * vb0, g[1] * vb1, g[2] * vb2, th2, QL1, QR1);
+          lr(ua[0] * vb0, ua[1] * vb1, ua[2] * vb2, th2, FL1, FR1);
+          const R Hnb = face2(tm_val(k8, 4, R()), tm_val(k8, 5, R()), QR1, FR1, cface);
+          tm_set(n8, 4, QL1); tm_set(n8, 5, FL1); tm_set(n8, 6, Hnb); tm_set(n8, 7, vb2);
+          tm_st_x(priv.field(fa), n8);
+          slot[0] = -(Hna - tm_val(k8, 2, R())) * sc_pi;
+          slot[256] = -(Hnb - tm_val(k8, 6, R())) * sc_pi;
+          slot += 2 * 256;
+        }
+      }
+      tm_wait_st();
+#undef P2_LD
+    } else {
+      // planes p and p-1 from global memory (L1 / L2), plane p-2 from the tile
       const R* __restrict__ pp[3] = {q2, q1, q0};
       // field m of plane p-2+t at the own column (t is a constant after unrolling)
 #define ETA_LD(t, m) ((ETILE && (t) == 0) ? town[(m) * MT_FST] : pp[t][(m) * FS])

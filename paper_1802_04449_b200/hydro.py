@@ -17,7 +17,7 @@ HYDRO_MEM_DEVICE, HYDRO_MEM_HOST = 0, 1
 SYMBOLS = ["hydro_workspace_bytes", "hydro_create", "hydro_load", "hydro_set_history", "hydro_read_history",
            "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_kernel", "hydro_destroy", "hydro_strerror",
            "hydro_freezeout_bytes", "hydro_freezeout_begin", "hydro_freezeout_slab", "hydro_freezeout_run",
-           "hydro_workspace_bytes_ext", "hydro_load_ext", "hydro_read_ext"]
+           "hydro_workspace_bytes_ext", "hydro_load_ext", "hydro_read_ext", "hydro_eos_e_of_temperature"]
 
 
 class hydro_grid(Structure):
@@ -91,6 +91,8 @@ def load_library():
     lib.hydro_load_ext.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int]
     lib.hydro_read_ext.restype = c_int
     lib.hydro_read_ext.argtypes = [c_void_p, c_void_p, c_void_p, c_int]
+    lib.hydro_eos_e_of_temperature.restype = c_int
+    lib.hydro_eos_e_of_temperature.argtypes = [POINTER(hydro_eos), c_double, POINTER(c_double)]
     lib.hydro_destroy.restype = None
     lib.hydro_destroy.argtypes = [c_void_p]
     lib.hydro_strerror.restype = ctypes.c_char_p
@@ -107,6 +109,27 @@ def _check(rc, what):
     if rc < 0:
         raise HydroError(f"{what}: {load_library().hydro_strerror(rc).decode()} (rc={rc})")
     return rc
+
+
+def make_eos(eos):
+    """hydro_eos from an inputs.conformal_eos() / crossover_table() dict; returns (struct, keep-alive arrays)."""
+    e = hydro_eos()
+    e.kind, e.n, e.e_min, e.e_max, e.c_sb = int(eos["kind"]), int(eos["n"]), float(eos["e_min"]), \
+        float(eos["e_max"]), float(eos["c_sb"])
+    P = None if eos["P"] is None else np.ascontiguousarray(eos["P"], dtype=np.float64)
+    T = None if eos["T"] is None else np.ascontiguousarray(eos["T"], dtype=np.float64)
+    e.P = None if P is None else P.ctypes.data_as(POINTER(c_double))
+    e.T = None if T is None else T.ctypes.data_as(POINTER(c_double))
+    return e, (P, T)
+
+
+def eos_e_of_T(eos, T_frz: float) -> float:
+    """hydro_eos_e_of_temperature: the energy density with temperature T_frz (GeV) -- a constant-T_f freeze-out surface is the
+    constant-e surface at this value.  Host arithmetic of the library; needs no device."""
+    e, keep = make_eos(eos)
+    out = c_double(0.0)
+    _check(load_library().hydro_eos_e_of_temperature(byref(e), float(T_frz), byref(out)), "hydro_eos_e_of_temperature")
+    return out.value
 
 
 def make_grid(nx, ny, nz, dx, dy, deta, bc=(0, 0, 0), geometry=0):

@@ -107,3 +107,19 @@ def test_create_refuses_a_host_workspace():
     h = c_void_p()
     assert lib.hydro_create(byref(h), byref(g), 0.01, 0.6, byref(e), 0.1, byref(o)) == -1
     assert not h.value
+
+
+def test_eos_e_of_T_inverts_the_oracle_temperature(conformal, crossover):
+    """hydro_eos_e_of_temperature (host arithmetic of the library, used for constant-T_f freeze-out) against the
+    ORACLE's T(e): e -> T_oracle(e) -> e(T) must return e, inside the table, below it, above it and for EOSI."""
+    import numpy as np
+    from oracle import Oracle
+    from paper_1802_04449_b200.hydro import eos_e_of_T
+    for eos in (conformal, crossover):
+        o = Oracle(1, 1, 1, 1, 1, 1, 0.1, 1.0, eos, 0.0)
+        for e in (3e-5, 1e-4, 0.0123, 0.6, 5.0, 77.7, 999.0, 4000.0):
+            T = o.eos(e)[2]
+            assert abs(eos_e_of_T(eos, T) / e - 1) < 1e-10, (eos["kind"], e)
+    # a temperature commonly used for the switch to hadrons sits in the crossover region of the synthetic table
+    e137 = eos_e_of_T(crossover, 0.137)
+    assert 0.05 < e137 < 2.0
