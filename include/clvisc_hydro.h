@@ -73,7 +73,7 @@ typedef struct {
  * count of the table root-find (<= 0: default 6); stream: a cudaStream_t (NULL = legacy default
  * stream); workspace: DEVICE memory of the current device, at least hydro_workspace_bytes(), 256-byte aligned (a host
  * pointer or memory of another GPU is refused with HYDRO_EINVAL).
- * kernel: 0 = default (the fastest one as measured on B200: 4 in both precisions);
+ * kernel: 0 = default (the fastest one as measured on B200: 4 from 5e5 cells on, 2 for smaller grids, both precisions);
  * 4 = marching per-cell kernel (hydro_stage_march.cuh): kernel 2's store and x / y flux code, but a block walks along
  * eta_s and forms every eta_s slope and face once, with the per-column pipeline state in tensor memory;
  * 2 = per-cell fused kernel on the extended 19-word state (hydro_stage_fused.cuh); 3 = tile kernel

@@ -49,10 +49,16 @@ struct Layout {
   size_t off_diag, off_eos, off_buf[3], off_gstar, total;
 };
 
-// kernel 0 = the fastest one as measured on B200 at 301x301x201 (round 2): the marching per-cell
-// kernel (4) in both precisions: fp64 11.8 ms per step against 14.4 (kernel 2) and 15.7 (kernel 3); fp32 6.3 against
-// 7.5 and 8.0.
-static int resolve_kernel(int kernel, int precision) { (void)precision; return kernel != 0 ? kernel : 4; }
+// kernel 0 = the fastest one as measured on B200 (round 2, profiles/round2_bench.md): the marching
+// per-cell kernel (4) from about 5e5 cells on (301x301x201: fp64 11.8 ms per step against 14.4 for kernel 2 and 15.7 for
+// kernel 3, fp32 6.05 against 7.5 and 8.0; 201x201x105: 3.04 against 3.46 ms); below that a block that walks along eta_s
+// leaves SMs idle and the per-cell kernel (2) wins (40x36x24: 0.063 against 0.111 ms; 33x33x17 ideal: 0.84 against 1.96 ms
+// for 40 steps).  Kernels 2 and 4 share the field store, so the choice does not change the workspace.
+static int resolve_kernel(int kernel, int precision, long long cells = 1ll << 40) {
+  (void)precision;
+  if (kernel != 0) return kernel;
+  return cells >= 500000 ? 4 : 2;
+}
 
 static bool make_layout(const hydro_grid* g, int precision, double eta_s, int kernel, Layout* L, bool ext = false) {
   if (!g || g->nx < 1 || g->ny < 1 || g->nz < 1) return false;
@@ -823,7 +829,7 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   if (!c) return HYDRO_ENOMEM;
   c->grid = *grid; c->dtau = dtau; c->tau0 = tau0; c->eta_s = eta_over_s;
   c->precision = opts->precision; c->visc = eta_over_s > 0.0 ? 1 : 0;
-  c->kernel = resolve_kernel(opts->kernel, opts->precision);
+  c->kernel = resolve_kernel(opts->kernel, opts->precision, (long long)grid->nx * grid->ny * grid->nz);
   c->strict = opts->strict_eq53 ? 1 : 0;
   c->ext = ext ? 1 : 0; c->zeta_s = ext ? opts->zeta_over_s : 0.0;
   if (ext) c->kernel = 2;
