@@ -243,13 +243,13 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
     const int k = p - 2;
     const bool centre = p >= kc0 + 2;                      // block-uniform
     if (CLV_MARCH_SYNC && !TILE) __syncthreads();
+    const R* __restrict__ q2 = in + (long long)bmap(p - 2, a.nz, a.bc[2]) * a.sz + col;    // plane p-2 (= k)
+    const R* __restrict__ q1 = in + (long long)bmap(p - 1, a.nz, a.bc[2]) * a.sz + col;
+    const R* __restrict__ q0 = in + (long long)bmap(p, a.nz, a.bc[2]) * a.sz + col;
     if (ETILE) {
       asm volatile("cp.async.wait_all;" ::: "memory");
       __syncthreads();                                     // tile(p-2) complete and visible
     }
-    const R* __restrict__ q2 = in + (long long)bmap(p - 2, a.nz, a.bc[2]) * a.sz + col;    // plane p-2 (= k)
-    const R* __restrict__ q1 = in + (long long)bmap(p - 1, a.nz, a.bc[2]) * a.sz + col;
-    const R* __restrict__ q0 = in + (long long)bmap(p, a.nz, a.bc[2]) * a.sz + col;
     if (CLV_MARCH_PF && p + 1 <= kc1 + 1 && (lane & (sizeof(R) == 8 ? 15 : 31)) == 0) {
       const R* __restrict__ qn = in + (long long)bmap(p + 1, a.nz, a.bc[2]) * a.sz + col;
 #pragma unroll
@@ -422,6 +422,8 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
       }
       if (USE_PI) {
         R* slot = &sS[tid];
+        // planes p-1 and p of the next trip's two fields are loaded one trip ahead (they come from L2 more often than not)
+        R nxt[2][2] = {{ETA_LD(1, F_PI), ETA_LD(1, F_PI + 1)}, {ETA_LD(2, F_PI), ETA_LD(2, F_PI + 1)}};
 #pragma unroll 1
         for (int t = 0; t < 5; ++t) {
           const int fa = F_PI + 2 * t;
@@ -429,9 +431,14 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
           priv.get(fa, QLa, FLa, Ha);
           priv.get(fa + 1, QLb, FLb, Hb);
           R qa[3], fa_[3], qb[3], fb[3];
+          const R cur[2][2] = {{nxt[0][0], nxt[0][1]}, {nxt[1][0], nxt[1][1]}};
+          if (t < 4) {
+            nxt[0][0] = ETA_LD(1, fa + 2); nxt[0][1] = ETA_LD(1, fa + 3);
+            nxt[1][0] = ETA_LD(2, fa + 2); nxt[1][1] = ETA_LD(2, fa + 3);
+          }
 #pragma unroll
           for (int s = 0; s < 3; ++s) {
-            const R va = ETA_LD(s, fa), vb = ETA_LD(s, fa + 1);
+            const R va = s == 0 ? ETA_LD(0, fa) : cur[s - 1][0], vb = s == 0 ? ETA_LD(0, fa + 1) : cur[s - 1][1];
             qa[s] = g[s] * va; fa_[s] = ua[s] * va;
             qb[s] = g[s] * vb; fb[s] = ua[s] * vb;
           }
@@ -495,6 +502,37 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
 #pragma unroll
       for (int n = 0; n < 4; ++n) grad[m][n] = R(0);
     const R sc_x = R(0.5) * a.scale[0], sc_y = R(0.5) * a.scale[1], sc_n = R(0.5) * a.scale[2];
+    // operands of the stage tail that come from global memory (state n / history / u*^tau at the cell, u~ of planes k+-1):
+    // issued here, ahead of the tile barrier and the refill, so that their latency runs behind both
+    const long long c = (long long)k * a.sz + col;
+    const long long cg = (long long)k * a.ny * a.gp + cg0;
+    if (MODE == 2) {
+      const R* __restrict__ sn = a.sn + c;
+      cn_.e = sn[0];
+      cn_.u[1] = sn[sf]; cn_.u[2] = sn[2 * sf]; cn_.u[3] = sn[3 * sf];
+      cn_.u[0] = sn[OX + X_G * FS];
+      cn_.P = sn[OX + X_P * FS];
+#pragma unroll
+      for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
+    }
+    R up3[3] = {R(0), R(0), R(0)};
+    R gst = R(1);
+    if (USE_PI) {
+      if (MODE == 1) {
+        const R* __restrict__ up = a.uprev + c;
+        up3[0] = up[0]; up3[1] = up[sf]; up3[2] = up[2 * sf];
+      } else {
+        gst = a.gstar[cg];
+      }
+    }
+
+    if (USE_PI) {      // eta_s row: planes k-1 and k+1 of the own column
+      const R* __restrict__ zm = in + (long long)bmap(k - 1, a.nz, a.bc[2]) * a.sz + col;
+      grad[3][0] = (q1[OX + X_G * FS] - zm[OX + X_G * FS]) * sc_n;
+      grad[3][1] = (q1[sf] - zm[sf]) * sc_n;
+      grad[3][2] = (q1[2 * sf] - zm[2 * sf]) * sc_n;
+      grad[3][3] = (q1[3 * sf] - zm[3 * sf]) * sc_n;
+    }
     if (TILE) {
       constexpr int OXT = NF * MT_FST;
       cc.e = town[0];
@@ -536,35 +574,6 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
         }
       }
     }
-    if (USE_PI) {      // eta_s row: planes k-1 and k+1 of the own column
-      const R* __restrict__ zm = in + (long long)bmap(k - 1, a.nz, a.bc[2]) * a.sz + col;
-      grad[3][0] = (q1[OX + X_G * FS] - zm[OX + X_G * FS]) * sc_n;
-      grad[3][1] = (q1[sf] - zm[sf]) * sc_n;
-      grad[3][2] = (q1[2 * sf] - zm[2 * sf]) * sc_n;
-      grad[3][3] = (q1[3 * sf] - zm[3 * sf]) * sc_n;
-    }
-    const long long c = (long long)k * a.sz + col;
-    const long long cg = (long long)k * a.ny * a.gp + cg0;
-    if (MODE == 2) {
-      const R* __restrict__ sn = a.sn + c;
-      cn_.e = sn[0];
-      cn_.u[1] = sn[sf]; cn_.u[2] = sn[2 * sf]; cn_.u[3] = sn[3 * sf];
-      cn_.u[0] = sn[OX + X_G * FS];
-      cn_.P = sn[OX + X_P * FS];
-#pragma unroll
-      for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
-    }
-    R up3[3] = {R(0), R(0), R(0)};
-    R gst = R(1);
-    if (USE_PI) {
-      if (MODE == 1) {
-        const R* __restrict__ up = a.uprev + c;
-        up3[0] = up[0]; up3[1] = up[sf]; up3[2] = up[2 * sf];
-      } else {
-        gst = a.gstar[cg];
-      }
-    }
-
     // ---- sources, stage update, root-find, limiter (hydro_stage_update.cuh) -----------------------------------------
     unsigned flags = 0;
     Cell<R> nw;
