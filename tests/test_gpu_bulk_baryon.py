@@ -131,3 +131,29 @@ def test_extension_is_refused_where_it_does_not_exist(crossover):
         from_config(small_parton_config(eta_over_s=0.0), crossover, bulk_baryon=1)
     with pytest.raises(HydroError):
         from_config(cfg, crossover).read_ext()
+
+
+def test_freezeout_finder_on_an_extended_context(crossover):
+    """The freeze-out finder (8(f)-1) reads e, u~, pi~ of a 16-word context through the same read path: keys bit-exact and
+    rows to 1e-8 against oracle/freezeout.py fed with the extended oracle's evolution."""
+    from oracle.freezeout import surface_elements
+    cfg = small_parton_config(eta_over_s=0.08, moving=True)
+    T, _ = inputs.ic_partons(cfg, inputs.seed_for(3))
+    nb0 = 0.3 * T[0]
+    o = ext_oracle(cfg, crossover)
+    o.load_ext(T, None, None, nb0)
+    e_frz = 0.35 * float(o.read()[0].max())
+    g = gpu(cfg, crossover)
+    g.load_ext(T, None, None, nb0)
+    g.freezeout_begin(e_frz, capacity=20000)
+    snap = o.read()
+    o.step(4); g.step(4)
+    nxt = o.read()
+    ok, orows = surface_elements(snap, nxt, cfg.tau0, cfg.tau0 + 4 * cfg.dtau, 0, (cfg.dx, cfg.dy, cfg.deta), e_frz)
+    n, hot = g.freezeout_slab()
+    keys, rows = g.freezeout_elements()
+    keys, rows = keys.cpu().numpy(), rows.cpu().numpy()
+    order = np.argsort(keys)
+    assert n == len(ok) and np.array_equal(keys[order], ok)
+    scale = np.maximum(np.abs(orows).max(axis=0), 1e-300)
+    assert (np.abs(rows[order] - orows).max(axis=0) / scale).max() < 1e-8
