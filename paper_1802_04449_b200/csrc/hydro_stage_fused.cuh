@@ -146,13 +146,14 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 #endif
 // KT flux difference (Eq.40-44) of every evolved field along axis AX from the five-point star pp[0..4] of the extended
 // state (pp[2] = the cell itself).  T fields: S[0..3] -= ...; pi fields: the thread-private shared-memory slots
-// slot0[m * 256] (INIT: first axis, "=" instead of "-=").  cfl = c_a h / Delta_a of the cell.  Shared by the per-cell
+// slot0[m * SSTR] (SSTR = threads per block; INIT: first axis, "=" instead of "-=").  cfl = c_a h / Delta_a of the cell.  Shared by the per-cell
 // kernel (three axes) and the marching kernel (x and y; hydro_stage_march.cuh).  FSTR = element stride between the
 // fields of a point (32 in the blocked global store; the plane size of a shared-memory tile).
 // EXT: two more pi-like fields follow the ten pi components -- the bulk pressure Pi (Q = u^tau Pi,
 // F_a = u^a Pi, Eq.30) and the net-baryon density n (Q_N / tau = n u^tau, F_a / tau = n u^a, Eq.28; the factor tau is
 // applied by the stage tail) -- and Pi adds to the pressure in the T fields (A28).
-template <typename R, bool USE_PI, int AX, bool INIT, int OX, int FSTR = FS, bool EXT = false, typename A, int NS>
+template <typename R, bool USE_PI, int AX, bool INIT, int OX, int FSTR = FS, bool EXT = false, int SSTR = 256, typename A,
+          int NS>
 __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ const (&pp)[5], R th2, R tf, R (&S)[NS],
                                           R* slot0, R& cfl) {
   constexpr int NTRIP = (EXT && USE_PI) ? 6 : 5;      // pi-like fields, two per trip
@@ -258,8 +259,8 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
         const F2 d = kt_div2_2(q, f, cl2, ncr2, th22);
         const R da = R(d.x) * sc_pi, db = R(d.y) * sc_pi;
         slot[0] = INIT ? -da : slot[0] - da;
-        slot[256] = INIT ? -db : slot[256] - db;
-        slot += 2 * 256;
+        slot[SSTR] = INIT ? -db : slot[SSTR] - db;
+        slot += 2 * SSTR;
       }
     } else {
 #pragma unroll 1
@@ -280,8 +281,8 @@ __device__ __forceinline__ void axis_flux(const A& a, const R* __restrict__ cons
       const R da = kt_div2(qa, fa, cl, cr, th2) * sc_pi;
       const R db = kt_div2(qb, fb, cl, cr, th2) * sc_pi;
       slot[0] = INIT ? -da : slot[0] - da;
-      slot[256] = INIT ? -db : slot[256] - db;
-      slot += 2 * 256;
+      slot[SSTR] = INIT ? -db : slot[SSTR] - db;
+      slot += 2 * SSTR;
     }
     }
   }

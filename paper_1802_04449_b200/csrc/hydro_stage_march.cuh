@@ -48,7 +48,12 @@ namespace clv {
 #define CLV_MARCH_PF_TAIL 0    // 1: L1 prefetch of what the stage tail reads at the cell (state n / history / u*^tau / plane
                                // k-1); measured neutral (11.84 vs 11.75 ms fp64), off
 #endif
-constexpr int MT_SX = 36, MT_SY = 12, MT_FST = MT_SX * MT_SY;      // tile extents and field stride (elements)
+#ifndef CLV_MARCH_TY
+#define CLV_MARCH_TY 8         // rows of cells per block (one warp per row)
+#endif
+constexpr int MTY = CLV_MARCH_TY, MT_NTHR = 32 * MTY;
+constexpr int MT_SX = 36, MT_SY = MTY + 4, MT_FST = MT_SX * MT_SY;      // tile extents and field stride (elements)
+constexpr int MT_NSLOT = (MT_FST + MT_NTHR - 1) / MT_NTHR;              // tile points copied per thread
 
 __device__ __forceinline__ void cp_async_elem(double* dst_smem, const double* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
@@ -130,7 +135,8 @@ struct MarchTmem {
   static constexpr int W = sizeof(R) / 4;
   static constexpr int NVAL = 14 * 4 + 3;
   static constexpr int COLS_PER_THREAD = NVAL * W;                       // 118 (fp64) / 59 (fp32)
-  static constexpr int ALLOC_COLS = 2 * COLS_PER_THREAD <= 128 ? 128 : 256;
+  static constexpr int WPQ = (MTY + 3) / 4;                              // warps per lane quadrant
+  static constexpr int ALLOC_COLS = WPQ * COLS_PER_THREAD <= 64 ? 64 : (WPQ * COLS_PER_THREAD <= 128 ? 128 : (WPQ * COLS_PER_THREAD <= 256 ? 256 : 512));
   unsigned base;
   __device__ __forceinline__ void init(unsigned tmem_base, int warp) {
     base = tmem_base + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)((warp >> 2) * COLS_PER_THREAD);
@@ -156,20 +162,21 @@ template <int N, int M> __device__ __forceinline__ void tm_wait_ld_x(TmWords<N>&
 #define CLV_MARCH_MINB32 3      // fp32 blocks per SM: 3 (<= 85 registers) measured 6.28 ms per step against 6.8 with 2
 #endif
 template <typename R, bool VISC, int MODE, bool TILE>
-__global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) stage_march_kernel(const StageArgs<R> a, const int chunk) {
+__global__ void __launch_bounds__(MT_NTHR, ((sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2) * 8 / MTY > 0 ? (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2) * 8 / MTY : 1))
+stage_march_kernel(const StageArgs<R> a, const int chunk) {
   static_assert(MODE == 1 || MODE == 2, "the bootstrap (MODE 0) runs in the per-cell kernel");
   constexpr bool USE_PI = VISC;
   constexpr int NF = VISC ? 14 : 4;
   constexpr int OX = NF * FS;
   const int lane = threadIdx.x, row = threadIdx.y, tid = row * 32 + lane;
-  const int i = blockIdx.x * 32 + lane, j = blockIdx.y * 8 + row;
+  const int i = blockIdx.x * 32 + lane, j = blockIdx.y * MTY + row;
   const bool active = (i < a.nx) && (j < a.ny);
   const int ic = active ? i : 0, jc = active ? j : 0;
   const int kc0 = blockIdx.z * chunk, kc1 = min(kc0 + chunk, a.nz);
   constexpr int sf = FS;
   const R* __restrict__ in = a.in;
 
-  __shared__ R sS[USE_PI ? 10 * 256 : 1];
+  __shared__ R sS[USE_PI ? 10 * MT_NTHR : 1];
   __shared__ unsigned s_tmem;
   extern __shared__ __align__(16) unsigned char tile_raw[];      // TILE: R tile[NF + 5][12][36]
   R* const tile = reinterpret_cast<R*>(tile_raw);
@@ -198,21 +205,21 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
   const long long cg0 = (long long)jc * a.gp + ic;
   // tile fill: this thread copies the points tid and tid + 256 of the 36 x 12 halo'd tile, all fields (boundary rule a11
   // applied to the source index, so the tile needs no special cases)
-  int tsrc[2];
+  int tsrc[MT_NSLOT];
 #pragma unroll
-  for (int s = 0; s < 2; ++s) {
-    const int pos = min(tid + 256 * s, MT_FST - 1);
+  for (int s = 0; s < MT_NSLOT; ++s) {
+    const int pos = min(tid + MT_NTHR * s, MT_FST - 1);
     const int r = pos / MT_SX, cx = pos - r * MT_SX;
-    tsrc[s] = (int)(bmap(blockIdx.y * 8 - 2 + r, a.ny, a.bc[1]) * a.sy +
+    tsrc[s] = (int)(bmap(blockIdx.y * MTY - 2 + r, a.ny, a.bc[1]) * a.sy +
                     xoff(bmap(blockIdx.x * 32 - 2 + cx, a.nx, a.bc[0]), a.blk));
   }
   auto fill_tile = [&](int kk) {
     const R* __restrict__ src = in + (long long)kk * a.sz;
 #pragma unroll
-    for (int s = 0; s < 2; ++s) {
-      if (s == 0 || tid + 256 < MT_FST) {
+    for (int s = 0; s < MT_NSLOT; ++s) {
+      if (tid + MT_NTHR * s < MT_FST) {
         const R* __restrict__ g0 = src + tsrc[s];
-        R* d0 = tile + (tid + 256 * s);
+        R* d0 = tile + (tid + MT_NTHR * s);
 #pragma unroll
         for (int m = 0; m < NFT; ++m) cp_async_elem(d0 + m * MT_FST, g0 + m * FS);
       }
@@ -295,15 +302,12 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
       const R cnew = q0[OX + X_CN * FS];
       R c1;
       {
-        W1 a0, a1, a2; W4 f0; W1 s3;
+        W1 a0, a1, a2, s0, s3;      // u~^tau, P, c_eta, e (field 0), u~^eta (field 3) of plane p-1
         tm_ld_x(priv.aux(0), a0); tm_ld_x(priv.aux(1), a1); tm_ld_x(priv.aux(2), a2);
-        tm_ld_x(priv.stash(0), s3);      // (reused below) e of plane p-1
-        tm_wait_ld_x(a0, a1); tm_wait_ld_x(a2, s3);
-        g[1] = tm_val(a0, 0, R()); Pp[1] = tm_val(a1, 0, R()); c1 = tm_val(a2, 0, R()); e3[1] = tm_val(s3, 0, R());
-        tm_ld_x(priv.stash(3), s3);
-        tm_wait_ld_x(s3);
+        tm_ld_x(priv.stash(0), s0); tm_ld_x(priv.stash(3), s3);
+        tm_wait_ld_x(a0, a1); tm_wait_ld_x(a2, s0); tm_wait_ld_x(s3);
+        g[1] = tm_val(a0, 0, R()); Pp[1] = tm_val(a1, 0, R()); c1 = tm_val(a2, 0, R()); e3[1] = tm_val(s0, 0, R());
         ua[1] = tm_val(s3, 0, R());
-        (void)f0;
       }
       const R cface = max_(c2, c1);
       cfl2 = c2 * a.h * a.scale[2];
@@ -374,8 +378,8 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
           tm_set(n8, 4, QL1); tm_set(n8, 5, FL1); tm_set(n8, 6, Hnb); tm_set(n8, 7, vb2);
           tm_st_x(priv.field(fa), n8);
           slot[0] = -(Hna - tm_val(k8, 2, R())) * sc_pi;
-          slot[256] = -(Hnb - tm_val(k8, 6, R())) * sc_pi;
-          slot += 2 * 256;
+          slot[MT_NTHR] = -(Hnb - tm_val(k8, 6, R())) * sc_pi;
+          slot += 2 * MT_NTHR;
         }
       }
       tm_wait_st();
@@ -452,8 +456,8 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
           const R Hnb = face2(QLb, FLb, QR1, FR1, cface);
           priv.put(fa + 1, QL1, FL1, Hnb);
           slot[0] = -(Hna - Ha) * sc_pi;
-          slot[256] = -(Hnb - Hb) * sc_pi;
-          slot += 2 * 256;
+          slot[MT_NTHR] = -(Hnb - Hb) * sc_pi;
+          slot += 2 * MT_NTHR;
         }
       }
       tm_wait_st();
@@ -476,22 +480,22 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
       const R* __restrict__ pp[5];
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = town + (t - 2);
-      axis_flux<R, USE_PI, 0, false, OXT, MT_FST>(a, pp, th2, tf, S, &sS[tid], cfl0);
+      axis_flux<R, USE_PI, 0, false, OXT, MT_FST, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl0);
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = town + (t - 2) * MT_SX;
-      axis_flux<R, USE_PI, 1, false, OXT, MT_FST>(a, pp, th2, tf, S, &sS[tid], cfl1);
+      axis_flux<R, USE_PI, 1, false, OXT, MT_FST, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl1);
     } else {
       const R* __restrict__ pp[5];
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = plane + offx[t];
-      axis_flux<R, USE_PI, 0, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl0);
+      axis_flux<R, USE_PI, 0, false, OX, FS, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl0);
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = plane + offy[t];
-      axis_flux<R, USE_PI, 1, false, OX>(a, pp, th2, tf, S, &sS[tid], cfl1);
+      axis_flux<R, USE_PI, 1, false, OX, FS, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl1);
     }
     if (USE_PI) {
 #pragma unroll
-      for (int m = 0; m < 10; ++m) S[4 + m] = sS[m * 256 + tid];
+      for (int m = 0; m < 10; ++m) S[4 + m] = sS[m * MT_NTHR + tid];
     }
 
     // ---- cell-centre state, velocity gradients ------------------------------------------------------------------------
@@ -628,8 +632,8 @@ __global__ void __launch_bounds__(256, (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2)) 
 
 // planes per chunk: whole waves of the resident blocks, against the two pipeline warm-up planes of a chunk
 inline int march_chunk(int nx, int ny, int nz, int nsm, int blocks_per_sm) {
-  const long long tiles = (long long)((nx + 31) / 32) * ((ny + 7) / 8);
-  const long long slots = (long long)blocks_per_sm * nsm;
+  const long long tiles = (long long)((nx + 31) / 32) * ((ny + MTY - 1) / MTY);
+  const long long slots = (long long)(blocks_per_sm * 8 / MTY > 0 ? blocks_per_sm * 8 / MTY : 1) * nsm;
   double best = -1.0;
   int best_chunk = nz;
   for (int nchunk = 1; nchunk <= nz; ++nchunk) {
@@ -654,8 +658,8 @@ cudaError_t launch_stage_march(const StageArgs<R>& a, int chunk, cudaStream_t st
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  dim3 block(32, 8, 1);
-  dim3 grid((a.nx + 31) / 32, (a.ny + 7) / 8, (a.nz + chunk - 1) / chunk);
+  dim3 block(32, MTY, 1);
+  dim3 grid((a.nx + 31) / 32, (a.ny + MTY - 1) / MTY, (a.nz + chunk - 1) / chunk);
   stage_march_kernel<R, VISC, MODE, TILE><<<grid, block, smem, stream>>>(a, chunk);
   return cudaGetLastError();
 }
