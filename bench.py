@@ -14,7 +14,8 @@ the fp64 run (BASELINE.json's metric names fp64 and fp32; the fp32 run of the sa
 Timing: W >= 3 warm-up steps, then exactly K steps between CUDA events recorded on the stream the
 kernels are launched on, stream-synchronised on both sides (barrier + max over ranks for N > 1).  The
 working set (3 state buffers of 14-19 fields x 146 MB) is far larger than the 126 MB L2, so no flush is needed.
-N > 1: one process per GPU, each evolving its own seeded event (replicas, no data-path collective);
+N > 1: one process per GPU, each evolving its own seeded event (replicas, no data-path collective; "scaling": "weak");
+`--decomp slabs` instead splits ONE event into eta_s slabs with a ghost-plane exchange after each stage ("strong").
 `--gpus N` without a torchrun environment re-executes itself under torch.distributed.run.
 """
 from __future__ import annotations
@@ -189,6 +190,9 @@ def main():
                     help="precision of the headline run (default 64; the other precision is the sub-record)")
     ap.add_argument("--kernel", type=int, default=0)
     ap.add_argument("--impl", default="b200", choices=("b200", "reference"))
+    ap.add_argument("--decomp", default="replicas", choices=("replicas", "slabs"),
+                    help="N > 1: one seeded event per rank (default, weak scaling, no data-path communication) or ONE "
+                         "event split into eta_s slabs with a ghost-plane exchange after each stage (strong scaling)")
     ap.add_argument("--grid", default="301,301,201", help="nx,ny,nz (default = configs[4])")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-steps", type=int, default=3, help="oracle steps of configs[4] for cpu_baseline (0 = skip)")
@@ -226,7 +230,9 @@ def main():
     if (nx, ny, nz) != (301, 301, 201):
         cfg.extra["partons"] = max(8, int(round(8000 * cfg.cells / (301.0 * 301 * 201))))
     eos = inputs.crossover_table()
-    T, _ = inputs.ic_partons(cfg, replicas.rank_seed(4, rank))     # one seeded event per rank
+    slab_mode = args.decomp == "slabs" and world > 1
+    # replicas: one seeded event per rank; slabs: every rank cuts its planes out of the same event
+    T, _ = inputs.ic_partons(cfg, replicas.rank_seed(4, 0 if slab_mode else rank))
     viscous = args.eta_over_s > 0
     counters = ncu_counters()
 
@@ -244,21 +250,30 @@ def main():
     def timed_run(precision):
         """Device-resident timing of K steps in one precision; returns the context and the record."""
         npdt = np.float64 if precision == 64 else np.float32
-        h = from_config(cfg, eos, precision=precision, kernel=args.kernel, device=f"cuda:{local}")
-        h.load(torch.from_numpy(T.astype(npdt)).to(dev))
-        h.step(args.warmup)
+        if slab_mode:
+            from paper_1802_04449_b200 import slabs
+            sl = slabs.Slab(cfg, eos, rank, world, precision=precision, kernel=args.kernel, device=f"cuda:{local}")
+            sl.load(T)
+            h = sl.h
+            step = lambda n: sl.step(n, slabs.exchange_dist)
+        else:
+            h = from_config(cfg, eos, precision=precision, kernel=args.kernel, device=f"cuda:{local}")
+            h.load(torch.from_numpy(T.astype(npdt)).to(dev))
+            step = h.step
+        step(args.warmup)
         barrier()
         l0 = h.launch_count()
         tw0 = time.perf_counter()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(h.stream)
-        h.step(args.steps)
+        step(args.steps)
         ev1.record(h.stream)
         barrier()
         windows.append((tw0, time.perf_counter()))
         ms_local = ev0.elapsed_time(ev1)
         launches = h.launch_count() - l0
-        value, ms = replicas.aggregate_rate(cfg.cells, args.steps, ms_local, world, dev)
+        # slabs: the N ranks share ONE event (cells of the whole grid once); replicas: N events
+        value, ms = replicas.aggregate_rate(cfg.cells / world if slab_mode else cfg.cells, args.steps, ms_local, world, dev)
         return h, dict(value=value, ms=ms, launches=int(launches), kernel=h.kernel(), diag=h.diag())
 
     h, main_rec = timed_run(args.precision)
@@ -277,7 +292,7 @@ def main():
         h.read(out=(e_h, u_h, None))      # the method's result: e and u^mu
 
     e2e = None
-    if args.e2e_steps > 0:
+    if args.e2e_steps > 0 and not slab_mode:
         e2e_step()
         barrier()
         t0 = time.perf_counter()
@@ -333,7 +348,8 @@ def main():
     d = main_rec["diag"]
     line = {"metric": METRIC, "value": main_rec["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": main_rec["ms"] / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32",
+            "scaling": "strong" if slab_mode else "weak", "vs_baseline": None,
+            "dtype": "f64" if args.precision == 64 else "f32",
             "data": "synthetic",
             "config": {"workload": f"configs[4]: {nx}x{ny}x{nz} cells, dx=dy=0.1 fm, deta=0.08, tau0=0.4, dtau=0.01, "
                                    f"eta/s={args.eta_over_s:g}, crossover EoS table (2000 nodes), {cfg.extra['partons']} seeded "
@@ -341,7 +357,8 @@ def main():
                        "cells": cfg.cells, "precision": args.precision, "kernel": main_rec["kernel"],
                        "kernel_requested": args.kernel,
                        "l2": "working set (3 state buffers) >> 126 MB L2, no flush needed",
-                       "parallelism": "1 event per GPU (replicas)" if world > 1 else "1 GPU"},
+                       "parallelism": ("1 event in %d eta_s slabs, ghost-plane exchange after each stage (NCCL send/recv)" % world
+                                       if slab_mode else ("1 event per GPU (replicas)" if world > 1 else "1 GPU"))},
             "roofline": roofline, "fp32" if args.precision == 64 else "fp64": second_rec,
             "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": main_rec["launches"], "clocks": clocks,
             "diag": {k: d[k] for k in ("tau", "step", "cfl", "e_max", "floored", "clamped", "pi_limited", "nan",

@@ -149,6 +149,23 @@ int hydro_read_history(hydro_ctx *ctx, void *u_prev, int mem);
  * Errors: HYDRO_ESTATE before hydro_load; HYDRO_ECUDA on a launch error. */
 int hydro_step(hydro_ctx *ctx, int n);
 
+/* ---- eta_s-slab decomposition --------------------------------------------------------------
+ * One event can be split into slabs of eta_s planes, one context per slab (one GPU each), each slab carrying two ghost
+ * planes per interior side and a zero-gradient boundary in its own eta_s: the stencil reaches two planes, so the results
+ * of a slab's interior planes are exactly those of the undivided grid as long as the ghost planes hold the neighbours'
+ * data when a stage reads them.  That takes one exchange after EACH stage, hence:
+ * hydro_stage: run ONE stage of the current RK2 step (1: state n -> state '; 2: -> state n+1, completes the step).
+ *   hydro_step(ctx, 1) == hydro_stage(ctx, 1); hydro_stage(ctx, 2).  HYDRO_ESTATE out of order; HYDRO_EINVAL for
+ *   kernel 3 or strict_eq53.
+ * hydro_plane_bytes: bytes of one eta_s plane of a state buffer (all fields, internal layout; 0 for kernel 3).
+ * hydro_planes: copy nk whole planes [k0, k0 + nk) of a state buffer out of (dir 0) or into (dir 1) the context.
+ *   which 0: the current state (state n; after a completed step state n+1); which 1: the stage-1 state '.
+ *   The layout is opaque: the bytes are only meant for the same planes of another context with the same nx, ny,
+ *   precision and viscosity (paper_1802_04449_b200/slabs.py).  Stream-ordered; host buffers synchronise. */
+int hydro_stage(hydro_ctx *ctx, int stage);
+size_t hydro_plane_bytes(const hydro_ctx *ctx);
+int hydro_planes(hydro_ctx *ctx, int which, int k0, int nk, void *buf, int dir, int mem);
+
 /* Read the state: e [nz][ny][nx], u = u~^mu [4][nz][ny][nx], pi = pi~ [10][nz][ny][nx]; any may be
  * NULL.  Synchronises the stream when mem == HYDRO_MEM_HOST. */
 int hydro_read(hydro_ctx *ctx, void *e, void *u, void *pi, int mem);

@@ -300,6 +300,7 @@ struct hydro_ctx {
   hydro_grid grid;
   double dtau, tau0, eta_s;
   int precision, visc, kernel, strict, ext;
+  int half;          // 1 between hydro_stage(1) and hydro_stage(2)
   double zeta_s;
   double theta, e_floor, xi, v_max, lambda1_hat, c_tau;
   int root_iters;
@@ -534,8 +535,9 @@ int do_bootstrap(hydro_ctx* c) {
   return c->visc ? launch_stage<R, true, 0>(c, a) : launch_stage<R, false, 0>(c, a);
 }
 
+// which: 0 = the whole RK2 step; 1 / 2 = one stage only (hydro_stage: blocked store, not with strict_eq53)
 template <typename R>
-int do_step(hydro_ctx* c) {
+int do_step(hydro_ctx* c, int which = 0) {
   const double tau_n = c->tau0 + (double)c->step * c->dtau, tau_1 = tau_n + c->dtau;
   const int slot = (int)(c->step & 1);
   R* cur = static_cast<R*>(c->buf[c->cur]);
@@ -582,15 +584,17 @@ int do_step(hydro_ctx* c) {
     c->launches += 2;
     rc = cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
   } else if (c->visc) {
-    rc = launch_stage<R, true, 1>(c, a1);
+    rc = which == 2 ? HYDRO_OK : launch_stage<R, true, 1>(c, a1);
     if (rc) return rc;
-    rc = launch_stage<R, true, 2>(c, a2);
+    if (which != 1) rc = launch_stage<R, true, 2>(c, a2);
   } else {
-    rc = launch_stage<R, false, 1>(c, a1);
+    rc = which == 2 ? HYDRO_OK : launch_stage<R, false, 1>(c, a1);
     if (rc) return rc;
-    rc = launch_stage<R, false, 2>(c, a2);
+    if (which != 1) rc = launch_stage<R, false, 2>(c, a2);
   }
   if (rc) return rc;
+  if (which == 1) { c->half = 1; return HYDRO_OK; }
+  c->half = 0;
   const int t = c->cur; c->cur = c->prev; c->prev = t;
   c->step += 1;
   return HYDRO_OK;
@@ -628,7 +632,7 @@ int do_load(hydro_ctx* c, const void* T, const void* pi, int mem, const void* Pi
     }
   }
   if (cudaMemsetAsync(c->diag, 0, sizeof(DiagDev), c->stream) != cudaSuccess) return HYDRO_ECUDA;
-  c->cur = 0; c->prev = 1; c->step = 0;
+  c->cur = 0; c->prev = 1; c->step = 0; c->half = 0;
   const unsigned nblk = (unsigned)((N + 255) / 256);
   if (c->L.soa) {
     SoaArgs<R> a = soa_args<R>(c);
@@ -902,9 +906,35 @@ int hydro_read_history(hydro_ctx* c, void* u_prev, int mem) {
   return c->precision == 64 ? do_history<double>(c, u_prev, mem, 1) : do_history<float>(c, u_prev, mem, 1);
 }
 
+int hydro_stage(hydro_ctx* c, int stage) {
+  if (!c || (stage != 1 && stage != 2)) return HYDRO_EINVAL;
+  if (!c->loaded || c->half != stage - 1) return HYDRO_ESTATE;      // stage 1, then stage 2
+  if (c->L.soa || c->strict) return HYDRO_EINVAL;
+  return c->precision == 64 ? do_step<double>(c, stage) : do_step<float>(c, stage);
+}
+
+size_t hydro_plane_bytes(const hydro_ctx* c) { return (c && !c->L.soa) ? (size_t)c->L.sz * c->L.elem : 0; }
+
+int hydro_planes(hydro_ctx* c, int which, int k0, int nk, void* buf, int dir, int mem) {
+  if (!c || !buf || (which != 0 && which != 1) || (dir != 0 && dir != 1) || nk < 1 || k0 < 0 || k0 + nk > c->grid.nz ||
+      (mem != HYDRO_MEM_DEVICE && mem != HYDRO_MEM_HOST))
+    return HYDRO_EINVAL;
+  if (!c->loaded) return HYDRO_ESTATE;
+  if (c->L.soa) return HYDRO_EINVAL;
+  char* base = static_cast<char*>(which == 0 ? c->buf[c->cur] : c->buf[2]) + (size_t)k0 * c->L.sz * c->L.elem;
+  const size_t bytes = (size_t)nk * c->L.sz * c->L.elem;
+  const cudaMemcpyKind kind = mem == HYDRO_MEM_DEVICE ? cudaMemcpyDeviceToDevice
+                                                      : (dir == 0 ? cudaMemcpyDeviceToHost : cudaMemcpyHostToDevice);
+  const cudaError_t e = dir == 0 ? cudaMemcpyAsync(buf, base, bytes, kind, c->stream)
+                                 : cudaMemcpyAsync(base, buf, bytes, kind, c->stream);
+  if (e != cudaSuccess) return HYDRO_ECUDA;
+  if (mem == HYDRO_MEM_HOST && cudaStreamSynchronize(c->stream) != cudaSuccess) return HYDRO_ECUDA;
+  return HYDRO_OK;
+}
+
 int hydro_step(hydro_ctx* c, int n) {
   if (!c || n < 0) return HYDRO_EINVAL;
-  if (!c->loaded) return HYDRO_ESTATE;
+  if (!c->loaded || c->half) return HYDRO_ESTATE;
   for (int s = 0; s < n; ++s) {
     const int rc = c->precision == 64 ? do_step<double>(c) : do_step<float>(c);
     if (rc) return rc;

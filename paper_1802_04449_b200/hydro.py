@@ -17,7 +17,8 @@ HYDRO_MEM_DEVICE, HYDRO_MEM_HOST = 0, 1
 SYMBOLS = ["hydro_workspace_bytes", "hydro_create", "hydro_load", "hydro_set_history", "hydro_read_history",
            "hydro_step", "hydro_read", "hydro_diag", "hydro_launch_count", "hydro_kernel", "hydro_destroy", "hydro_strerror",
            "hydro_freezeout_bytes", "hydro_freezeout_begin", "hydro_freezeout_slab", "hydro_freezeout_run",
-           "hydro_workspace_bytes_ext", "hydro_load_ext", "hydro_read_ext", "hydro_eos_e_of_temperature"]
+           "hydro_workspace_bytes_ext", "hydro_load_ext", "hydro_read_ext", "hydro_eos_e_of_temperature",
+           "hydro_stage", "hydro_plane_bytes", "hydro_planes"]
 
 
 class hydro_grid(Structure):
@@ -93,6 +94,12 @@ def load_library():
     lib.hydro_read_ext.argtypes = [c_void_p, c_void_p, c_void_p, c_int]
     lib.hydro_eos_e_of_temperature.restype = c_int
     lib.hydro_eos_e_of_temperature.argtypes = [POINTER(hydro_eos), c_double, POINTER(c_double)]
+    lib.hydro_stage.restype = c_int
+    lib.hydro_stage.argtypes = [c_void_p, c_int]
+    lib.hydro_plane_bytes.restype = c_size_t
+    lib.hydro_plane_bytes.argtypes = [c_void_p]
+    lib.hydro_planes.restype = c_int
+    lib.hydro_planes.argtypes = [c_void_p, c_int, c_int, c_int, c_void_p, c_int, c_int]
     lib.hydro_destroy.restype = None
     lib.hydro_destroy.argtypes = [c_void_p]
     lib.hydro_strerror.restype = ctypes.c_char_p
@@ -236,6 +243,34 @@ class Hydro:
     def step(self, n=1):
         with self._torch.cuda.device(self.device):
             _check(self._lib.hydro_step(self._h, int(n)), "hydro_step")
+
+    # -- eta_s-slab decomposition (hydro_stage / hydro_planes; paper_1802_04449_b200/slabs.py) ----------------
+    def stage(self, which):
+        """One stage of the current RK2 step: stage(1) then stage(2) is step(1)."""
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_stage(self._h, int(which)), "hydro_stage")
+
+    def plane_bytes(self) -> int:
+        return int(self._lib.hydro_plane_bytes(self._h))
+
+    def planes_get(self, which, k0, nk, host=False):
+        """nk whole eta_s planes of a state buffer (0: current state, 1: stage-1 state) as opaque bytes (uint8 tensor)."""
+        torch = self._torch
+        n = nk * self.plane_bytes()
+        buf = torch.empty(n, dtype=torch.uint8, device="cpu" if host else self.device)
+        with torch.cuda.device(self.device):
+            _check(self._lib.hydro_planes(self._h, int(which), int(k0), int(nk), c_void_p(buf.data_ptr()), 0,
+                                          HYDRO_MEM_HOST if host else HYDRO_MEM_DEVICE), "hydro_planes")
+        return buf
+
+    def planes_put(self, which, k0, buf):
+        """Write planes obtained from planes_get of a context with the same nx, ny, precision and viscosity."""
+        nk, rem = divmod(buf.numel(), self.plane_bytes())
+        if rem or buf.dtype != self._torch.uint8 or not buf.is_contiguous():
+            raise HydroError("planes_put: a contiguous uint8 tensor of whole planes is required")
+        with self._torch.cuda.device(self.device):
+            _check(self._lib.hydro_planes(self._h, int(which), int(k0), int(nk), c_void_p(buf.data_ptr()), 1,
+                                          HYDRO_MEM_DEVICE if buf.is_cuda else HYDRO_MEM_HOST), "hydro_planes")
 
     def _empty(self, shape, host, pinned=False):
         torch = self._torch
