@@ -101,7 +101,7 @@ typedef struct {
    * bulk pressure Pi and the net-baryon density n next to T^{tau mu} and pi^{mu nu} (readings A28-A32):
    *   T_f^{mu nu} = (e + P + Pi) u u - (P + Pi) g + pi;   d_mu(u^mu Pi) = -(Pi + zeta theta)/tau_Pi - Pi theta/3 with
    *   tau_Pi = tau_pi and zeta = zeta_over_s * s;   d~_mu(tau n u~^mu) = 0;   root-find with P + Pi;   |Pi| <= xi P.
-   * Viscous runs only, per-cell fused kernel (opts->kernel 0, 2 or 4; it runs kernel 2), not with strict_eq53; needs
+   * Viscous runs only, kernels 2 and 4 (opts->kernel 0, 2 or 4), not with strict_eq53; needs
    * hydro_workspace_bytes_ext(); state loaded / read with hydro_load_ext / hydro_read_ext.  0 = off (the paper's setting,
    * "bulk viscosity and net baryon density are set to 0 in the current version"). */
   int bulk_baryon;

@@ -498,9 +498,13 @@ StageArgs<R> stage_args(const hydro_ctx* c, double tau_rhs, double tau_n, double
 template <typename R, bool VISC, int MODE>
 int launch_stage(hydro_ctx* c, const StageArgs<R>& a) {
   if constexpr (VISC) {
-    if (c->ext) {      // the 16-word cell runs in the per-cell fused kernel
-      launch_stage_fused<R, true, MODE, true>(a, c->stream);
+    if (c->ext) {      // the 16-word cell, kernels 4 (marching) and 2 (per-cell; also the bootstrap)
       c->launches += 1;
+      if constexpr (MODE != 0) {
+        if (c->kernel == 4)
+          return launch_stage_march<R, true, MODE, true>(a, c->march_chunk, c->stream) == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
+      }
+      launch_stage_fused<R, true, MODE, true>(a, c->stream);
       return cudaGetLastError() == cudaSuccess ? HYDRO_OK : HYDRO_ECUDA;
     }
   }
@@ -836,7 +840,6 @@ int hydro_create(hydro_ctx** out, const hydro_grid* grid, double dtau, double ta
   c->kernel = resolve_kernel(opts->kernel, opts->precision, (long long)grid->nx * grid->ny * grid->nz);
   c->strict = opts->strict_eq53 ? 1 : 0;
   c->ext = ext ? 1 : 0; c->zeta_s = ext ? opts->zeta_over_s : 0.0;
-  if (ext) c->kernel = 2;
   c->theta = opts->minmod_theta; c->e_floor = opts->e_floor; c->xi = opts->pi_limit_xi;
   c->v_max = opts->v_max > 0.0 ? opts->v_max : 0.999;   // gamma <= 22.4 (A7)
   c->root_iters = opts->root_iters > 0 ? opts->root_iters : 6;

@@ -142,10 +142,10 @@ template <int N> __device__ __forceinline__ void tm_set(TmWords<N>& v, int i, do
 }
 template <int N> __device__ __forceinline__ void tm_set(TmWords<N>& v, int i, float x) { v.w[i] = __float_as_uint(x); }
 
-template <typename R>
+template <typename R, int NFLD = 14>
 struct MarchTmem {
   static constexpr int W = sizeof(R) / 4;
-  static constexpr int NVAL = 14 * 4 + 3;
+  static constexpr int NVAL = NFLD * 4 + (NFLD == 14 ? 3 : 0);           // 16 fields (8(f)-3): no stash, no aux words
   static constexpr int COLS_PER_THREAD = NVAL * W;                       // 118 (fp64) / 59 (fp32)
   static constexpr int WPQ = (MTY + 3) / 4;                              // warps per lane quadrant
   static constexpr int ALLOC_COLS = WPQ * COLS_PER_THREAD <= 64 ? 64 : (WPQ * COLS_PER_THREAD <= 128 ? 128 : (WPQ * COLS_PER_THREAD <= 256 ? 256 : 512));
@@ -155,7 +155,7 @@ struct MarchTmem {
   }
   __device__ __forceinline__ unsigned field(int f) const { return base + (unsigned)(f * 4 * W); }      // 4 values of field f
   __device__ __forceinline__ unsigned stash(int f) const { return base + (unsigned)((f * 4 + 3) * W); }
-  __device__ __forceinline__ unsigned aux(int i) const { return base + (unsigned)((56 + i) * W); }   // 0 u~^tau, 1 P, 2 c_eta
+  __device__ __forceinline__ unsigned aux(int i) const { return base + (unsigned)((NFLD * 4 + i) * W); }   // 0 u~^tau, 1 P, 2 c_eta
   // three-value access (the build without the stash, CLV_MARCH_STASH = 0)
   __device__ __forceinline__ void get(int f, R& ql, R& fl, R& h) const { tm_ld3(field(f), ql, fl, h); }
   __device__ __forceinline__ void put(int f, R ql, R fl, R h) const {
@@ -173,12 +173,15 @@ template <int N, int M> __device__ __forceinline__ void tm_wait_ld_x(TmWords<N>&
 #ifndef CLV_MARCH_MINB32
 #define CLV_MARCH_MINB32 3      // fp32 blocks per SM: 3 (<= 85 registers) measured 6.28 ms per step against 6.8 with 2
 #endif
-template <typename R, bool VISC, int MODE, bool TILE>
+// EXT: the 16-word cell -- fields 14 (Pi) and 15 (n) ride along as two more pi-like fields.
+template <typename R, bool VISC, int MODE, bool TILE, bool EXT = false>
 __global__ void __launch_bounds__(MT_NTHR, ((sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2) * 8 / MTY > 0 ? (sizeof(R) == 4 ? CLV_MARCH_MINB32 : 2) * 8 / MTY : 1))
 stage_march_kernel(const StageArgs<R> a, const int chunk) {
   static_assert(MODE == 1 || MODE == 2, "the bootstrap (MODE 0) runs in the per-cell kernel");
   constexpr bool USE_PI = VISC;
-  constexpr int NF = VISC ? 14 : 4;
+  static_assert(!EXT || VISC, "the bulk / baryon extension rides on the viscous path");
+  constexpr int NF = VISC ? (EXT ? 16 : 14) : 4;
+  constexpr int NPI = EXT ? 12 : 10, NTRIP = NPI / 2;      // pi-like fields, two per trip
   constexpr int OX = NF * FS;
   const int lane = threadIdx.x, row = threadIdx.y, tid = row * 32 + lane;
   const int i = blockIdx.x * 32 + lane, j = blockIdx.y * MTY + row;
@@ -188,12 +191,12 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
   constexpr int sf = FS;
   const R* __restrict__ in = a.in;
 
-  __shared__ R sS[USE_PI ? 10 * MT_NTHR : 1];
+  __shared__ R sS[USE_PI ? NPI * MT_NTHR : 1];
   __shared__ unsigned s_tmem;
   extern __shared__ __align__(16) unsigned char tile_raw[];      // TILE: R tile[NF + 5][12][36]
   R* const tile = reinterpret_cast<R*>(tile_raw);
   constexpr int NFT = NF + X_COUNT;
-  using Priv = MarchTmem<R>;
+  using Priv = MarchTmem<R, EXT ? 16 : 14>;
   if (row == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)),
                  "r"((unsigned)Priv::ALLOC_COLS) : "memory");
@@ -280,7 +283,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
   const R sc_pi = R(0.5) * a.scale[2], sc_T = sc_pi * tf;
   R cflm0 = R(0), cflm1 = R(0), cflm2 = R(0), emax = R(0);
 
-  constexpr bool STASH = (CLV_MARCH_STASH == 1) || (CLV_MARCH_STASH == 2 && sizeof(R) == 4);
+  constexpr bool STASH = !EXT && ((CLV_MARCH_STASH == 1) || (CLV_MARCH_STASH == 2 && sizeof(R) == 4));
   if constexpr (STASH) {   // the stash starts with plane kc0-1
     const R* __restrict__ qm = in + (long long)bmap(kc0 - 1, a.nz, a.bc[2]) * a.sz + col;
     TmWords<Priv::W> v;
@@ -328,9 +331,9 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
       }
     }
 
-    R S[14];
+    R S[16];
 #pragma unroll
-    for (int m = 0; m < 14; ++m) S[m] = R(0);
+    for (int m = 0; m < 16; ++m) S[m] = R(0);
     R cfl2;
     // ---- eta_s pipeline step: slope of cell p-1, face p-3/2, flux difference of cell p-2 ---------------------------
     if constexpr (STASH) {
@@ -445,6 +448,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
 #pragma unroll
         for (int t = 0; t < 3; ++t) {
           Pp[t] = ETA_LD(t, NF + X_P);
+          if (EXT) Pp[t] += ETA_LD(t, F_PI + 10);      // P + Pi (A28)
           const R w = ETA_LD(t, 0) + Pp[t];
           wq[t] = w * g[t]; wa[t] = w * ua[t];
         }
@@ -474,14 +478,14 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
         // planes p-1 and p of the next trip's two fields are loaded one trip ahead (they come from L2 more often than not)
         R nxt[2][2] = {{ETA_LD(1, F_PI), ETA_LD(1, F_PI + 1)}, {ETA_LD(2, F_PI), ETA_LD(2, F_PI + 1)}};
 #pragma unroll 1
-        for (int t = 0; t < 5; ++t) {
+        for (int t = 0; t < NTRIP; ++t) {
           const int fa = F_PI + 2 * t;
           R QLa, FLa, Ha, QLb, FLb, Hb;
           priv.get(fa, QLa, FLa, Ha);
           priv.get(fa + 1, QLb, FLb, Hb);
           R qa[3], fa_[3], qb[3], fb[3];
           const R cur[2][2] = {{nxt[0][0], nxt[0][1]}, {nxt[1][0], nxt[1][1]}};
-          if (t < 4) {
+          if (t < NTRIP - 1) {
             nxt[0][0] = ETA_LD(1, fa + 2); nxt[0][1] = ETA_LD(1, fa + 3);
             nxt[1][0] = ETA_LD(2, fa + 2); nxt[1][1] = ETA_LD(2, fa + 3);
           }
@@ -525,22 +529,22 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
       const R* __restrict__ pp[5];
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = town + (t - 2);
-      axis_flux<R, USE_PI, 0, false, OXT, MT_FST, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl0);
+      axis_flux<R, USE_PI, 0, false, OXT, MT_FST, EXT, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl0);
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = town + (t - 2) * MT_SX;
-      axis_flux<R, USE_PI, 1, false, OXT, MT_FST, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl1);
+      axis_flux<R, USE_PI, 1, false, OXT, MT_FST, EXT, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl1);
     } else {
       const R* __restrict__ pp[5];
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = plane + offx[t];
-      axis_flux<R, USE_PI, 0, false, OX, FS, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl0);
+      axis_flux<R, USE_PI, 0, false, OX, FS, EXT, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl0);
 #pragma unroll
       for (int t = 0; t < 5; ++t) pp[t] = plane + offy[t];
-      axis_flux<R, USE_PI, 1, false, OX, FS, false, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl1);
+      axis_flux<R, USE_PI, 1, false, OX, FS, EXT, MT_NTHR>(a, pp, th2, tf, S, &sS[tid], cfl1);
     }
     if (USE_PI) {
 #pragma unroll
-      for (int m = 0; m < 10; ++m) S[4 + m] = sS[m * MT_NTHR + tid];
+      for (int m = 0; m < NPI; ++m) S[4 + m] = sS[m * MT_NTHR + tid];
     }
 
     // ---- cell-centre state, velocity gradients ------------------------------------------------------------------------
@@ -563,6 +567,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
       cn_.P = sn[OX + X_P * FS];
 #pragma unroll
       for (int m = 0; m < 10; ++m) cn_.pi[m] = VISC ? sn[(F_PI + m) * FS] : R(0);
+      cn_.Pi = EXT ? sn[(F_PI + 10) * FS] : R(0); cn_.nb = EXT ? sn[(F_PI + 11) * FS] : R(0);
     }
     R up3[3] = {R(0), R(0), R(0)};
     R gst = R(1);
@@ -590,6 +595,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
       cc.P = town[OXT + X_P * MT_FST];
 #pragma unroll
       for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? town[(F_PI + m) * MT_FST] : R(0);
+      cc.Pi = EXT ? town[(F_PI + 10) * MT_FST] : R(0); cc.nb = EXT ? town[(F_PI + 11) * MT_FST] : R(0);
       if (USE_PI) {
         grad[1][0] = (town[OXT + X_G * MT_FST + 1] - town[OXT + X_G * MT_FST - 1]) * sc_x;
         grad[2][0] = (town[OXT + X_G * MT_FST + MT_SX] - town[OXT + X_G * MT_FST - MT_SX]) * sc_y;
@@ -610,6 +616,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
       cc.P = pc[OX + X_P * FS];
 #pragma unroll
       for (int m = 0; m < 10; ++m) cc.pi[m] = USE_PI ? pc[(F_PI + m) * FS] : R(0);
+      cc.Pi = EXT ? pc[(F_PI + 10) * FS] : R(0); cc.nb = EXT ? pc[(F_PI + 11) * FS] : R(0);
       if (USE_PI) {
 #pragma unroll
         for (int ax = 0; ax < 2; ++ax) {
@@ -627,7 +634,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
     unsigned flags = 0;
     Cell<R> nw;
     R cs2_new;
-    stage_update<R, VISC, MODE>(a, S, cc, cn_, grad, up3, gst, nw, cs2_new, flags);
+    stage_update<R, VISC, MODE, EXT>(a, S, cc, cn_, grad, up3, gst, nw, cs2_new, flags, tf);
 
     if (active) {
       R* __restrict__ out = a.out + c;
@@ -637,6 +644,7 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
       if (VISC) {
 #pragma unroll
         for (int m = 0; m < 10; ++m) out[(F_PI + m) * FS] = nw.pi[m];
+        if (EXT) { out[(F_PI + 10) * FS] = nw.Pi; out[(F_PI + 11) * FS] = nw.nb; }
         if (MODE == 1) a.gstar[cg] = gst;
       }
       out[OX + X_P * FS] = nw.P; out[OX + X_G * FS] = nw.u[0];
@@ -691,21 +699,21 @@ inline int march_chunk(int nx, int ny, int nz, int nsm, int blocks_per_sm) {
   return best_chunk;
 }
 
-template <typename R, bool VISC, int MODE>
+template <typename R, bool VISC, int MODE, bool EXT = false>
 cudaError_t launch_stage_march(const StageArgs<R>& a, int chunk, cudaStream_t stream) {
   constexpr bool TILE = CLV_MARCH_TILE != 0;
-  constexpr int NFT = (VISC ? 14 : 4) + X_COUNT;
+  constexpr int NFT = (VISC ? (EXT ? 16 : 14) : 4) + X_COUNT;
   const size_t smem = TILE ? (size_t)NFT * MT_FST * sizeof(R) : 0;
   static bool configured = false;
   if (TILE && !configured) {
-    cudaError_t e = cudaFuncSetAttribute(stage_march_kernel<R, VISC, MODE, TILE>,
+    cudaError_t e = cudaFuncSetAttribute(stage_march_kernel<R, VISC, MODE, TILE, EXT>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
   dim3 block(32, MTY, 1);
   dim3 grid((a.nx + 31) / 32, (a.ny + MTY - 1) / MTY, (a.nz + chunk - 1) / chunk);
-  stage_march_kernel<R, VISC, MODE, TILE><<<grid, block, smem, stream>>>(a, chunk);
+  stage_march_kernel<R, VISC, MODE, TILE, EXT><<<grid, block, smem, stream>>>(a, chunk);
   return cudaGetLastError();
 }
 

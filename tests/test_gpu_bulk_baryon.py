@@ -31,8 +31,9 @@ def ext_errors(eos, oref, gref, e_ref):
     return dict(rel_Pi=float(np.max(np.abs(Pg - Po) / w)), rel_n=float(np.max(np.abs(ng - no) / np.maximum(np.abs(no), 1e-300))))
 
 
+@pytest.mark.parametrize("kernel", [2, 4])
 @pytest.mark.parametrize("precision", [64, 32])
-def test_small_event_with_bulk_and_baryon(crossover, precision):
+def test_small_event_with_bulk_and_baryon(crossover, precision, kernel):
     """Small moving viscous event (eta/s = 0.16, zeta/s = 0.03), initial Pi = -0.2 P(T^{tau tau}) (|Pi| < P also on the
     fast dilute rim, where T^{tau tau} >> e) and n = 0.3 T^{tau tau}: one step at the 1e-10 bar, 12 steps at 1e-7 (fp64);
     fp32 relative L2 of e <= 2e-4."""
@@ -42,8 +43,8 @@ def test_small_event_with_bulk_and_baryon(crossover, precision):
     o.load(T)
     Pi0, nb0 = -0.2 * pressure(crossover, o.read()[0]), 0.3 * T[0]      # P of the Pi-free root-find: an input recipe
     o.load_ext(T, None, Pi0, nb0)
-    g = gpu(cfg, crossover, precision=precision)
-    assert g.kernel() == 2
+    g = gpu(cfg, crossover, precision=precision, kernel=kernel)
+    assert g.kernel() == kernel
     dt = g.np_dtype
     g.load_ext(T.astype(dt), None, Pi0.astype(dt), nb0.astype(dt))
     # the load itself: root-find with Pi
@@ -108,7 +109,7 @@ def test_cartesian_box_conserves_baryon_number(crossover):
     T = np.stack([(e + P + Pb) * g2 - (P + Pb)] + [(e + P + Pb) * g2 * v[a] for a in range(3)]) + pi[:4]
     o = ext_oracle(cfg, crossover)
     o.load_ext(T, pi, Pb, nb)
-    g = gpu(cfg, crossover)
+    g = gpu(cfg, crossover, kernel=4)
     g.load_ext(T, pi, Pb, nb)
     N0 = (g.read_ext()[1] * g.read()[1][0]).sum()
     o.step(4); g.step(4)
