@@ -58,6 +58,12 @@ constexpr int MT_NSLOT = (MT_FST + MT_NTHR - 1) / MT_NTHR;              // tile 
 __device__ __forceinline__ void cp_async_elem(double* dst_smem, const double* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
 }
+__device__ __forceinline__ void cp_async_elem_hint(double* dst_smem, const double* src, unsigned long long pol) {
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(smem_u32(dst_smem)), "l"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem_hint(float* dst_smem, const float* src, unsigned long long pol) {
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 4, %2;" ::"r"(smem_u32(dst_smem)), "l"(src), "l"(pol) : "memory");
+}
 __device__ __forceinline__ void cp_async_elem(float* dst_smem, const float* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst_smem)), "l"(src) : "memory");
 }
@@ -98,6 +104,9 @@ __device__ __forceinline__ void stg_hint(double* p, double v, unsigned long long
 __device__ __forceinline__ void stg_hint(float* p, float v, unsigned long long pol) {
   asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v), "l"(pol) : "memory");
 }
+#ifndef CLV_MARCH_FILLHINT
+#define CLV_MARCH_FILLHINT 0     // 1: the tile fill (second and last read of a plane by this block) asks L2 not to keep the lines
+#endif
 #ifndef CLV_MARCH_PAIRS
 #define CLV_MARCH_PAIRS 0      // 1: tile fill in pairs of x-consecutive points (128-bit copies in fp64).  Measured at
                                // 301x301x201: 11.65-11.71 ms per step fp64 / 5.92 fp32 against 11.45 / 5.84 with one point per
@@ -248,6 +257,11 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
     offy[p] = (int)(bmap(jc + p - 2, a.ny, a.bc[1]) * a.sy + xoff(ic, a.blk));
   }
   const long long cg0 = (long long)jc * a.gp + ic;
+  constexpr bool L2H = (CLV_MARCH_L2HINT == 1) || (CLV_MARCH_L2HINT == 2 && sizeof(R) == 8);
+  const unsigned long long pol_keep = L2H ? l2_policy(true) : 0ull;
+  const unsigned long long pol_once = L2H ? l2_policy(false) : 0ull;
+#define LDK(ptr) (L2H ? ldg_hint((ptr), pol_keep) : *(ptr))
+#define LD1(ptr) (L2H ? ldg_hint((ptr), pol_once) : *(ptr))
   // tile fill (boundary rule a11 applied to the source index, so the tile needs no special cases).  The 36 x 12 points
   // are copied as 18 x 12 PAIRS of x-consecutive points, one pair per thread and field: the tile starts at an even x
   // (32 bx - 2), pairs never straddle an x-block of the store, so a pair is one aligned 16-byte (fp64) / 8-byte (fp32)
@@ -298,7 +312,10 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
           const R* __restrict__ g0 = src + tsrc[s];
           R* d0 = tile + (tid + MT_NTHR * s);
 #pragma unroll
-          for (int m = 0; m < NFT; ++m) cp_async_elem(d0 + m * MT_FST, g0 + m * FS);
+          for (int m = 0; m < NFT; ++m) {
+            if (CLV_MARCH_FILLHINT && L2H) cp_async_elem_hint(d0 + m * MT_FST, g0 + m * FS, pol_once);
+            else cp_async_elem(d0 + m * MT_FST, g0 + m * FS);
+          }
         }
       }
     }
@@ -308,11 +325,6 @@ stage_march_kernel(const StageArgs<R> a, const int chunk) {
   if (TILE) fill_tile(ETILE ? bmap(kc0 - 2, a.nz, a.bc[2]) : kc0);
   const R* const town = tile + (row + 2) * MT_SX + (lane + 2);      // own point inside a field plane of the tile
 
-  constexpr bool L2H = (CLV_MARCH_L2HINT == 1) || (CLV_MARCH_L2HINT == 2 && sizeof(R) == 8);
-  const unsigned long long pol_keep = L2H ? l2_policy(true) : 0ull;
-  const unsigned long long pol_once = L2H ? l2_policy(false) : 0ull;
-#define LDK(ptr) (L2H ? ldg_hint((ptr), pol_keep) : *(ptr))
-#define LD1(ptr) (L2H ? ldg_hint((ptr), pol_once) : *(ptr))
   const R tf = a.milne ? a.tau : R(1);
   const R th2 = R(2) * a.theta;
   const R sc_pi = R(0.5) * a.scale[2], sc_T = sc_pi * tf;
