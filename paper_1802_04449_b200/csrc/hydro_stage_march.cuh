@@ -19,7 +19,8 @@
 //     reads plane p-1 from there and only ONE plane per step comes from global memory (fp64: measured slower, off);
 //   * one block barrier per plane (two with the tile) keeps the 8 warps of a block on the same instruction-cache lines
 //     of the ~90 KB loop body: without it "no instruction" stalls are 1.8 warps per issue, with it 0.19.
-// Measured at 301x301x201 (profiles/round2_bench.md): 11.8 ms per step fp64, 6.1 ms fp32 (kernel 2: 14.4 / 7.5).
+//   * fp64 only: L2 eviction hints (keep the first read of a plane for the tile fill two steps later; stream the rest).
+// Measured at 301x301x201 (profiles/round2_bench.md): 11.3 ms per step fp64, 5.84 ms fp32 (kernel 2: 14.4 / 7.5).
 // Citations: KT scheme PAPER.md:193-213 (Eq.40-44); RK2 :225-239 (Eq.49-54).
 #pragma once
 #include "hydro_stage_fused.cuh"
